@@ -1,0 +1,136 @@
+"""ctypes front end of oracle/acm_oracle.c (TEST INFRASTRUCTURE, not the product).
+
+Mirrors the call list of include/acm.h with host (numpy) arrays so that one test
+harness can drive both the oracle and the CUDA library.  No arithmetic of the
+method lives here: every number comes out of acm_oracle.c.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(_build.build())
+        dp = C.POINTER(C.c_double)
+        ip = C.POINTER(C.c_int)
+        lib.oracle_create.argtypes = [C.POINTER(C.c_void_p)] + [C.c_int] * 5 + [C.c_double] * 7 + [dp, C.c_uint]
+        lib.oracle_destroy.argtypes = [C.c_void_p]
+        lib.oracle_destroy.restype = None
+        lib.oracle_init.argtypes = [C.c_void_p, dp, dp]
+        lib.oracle_step.argtypes = [C.c_void_p, C.c_int]
+        lib.oracle_fields.argtypes = [C.c_void_p, dp, dp, dp]
+        lib.oracle_phi_mass.argtypes = [C.c_void_p, dp]
+        lib.oracle_get_pdfs.argtypes = [C.c_void_p, dp, dp]
+        lib.oracle_set_pdfs.argtypes = [C.c_void_p, dp, dp]
+        lib.oracle_lattice.argtypes = [C.c_int, ip, dp, ip, dp, dp, ip]
+        lib.oracle_fd.argtypes = [C.c_void_p, C.c_int, dp, dp, dp]
+        lib.oracle_set_threads.argtypes = [C.c_int]
+        _lib = lib
+    return _lib
+
+
+def _dp(a):
+    return None if a is None else a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def set_threads(n: int) -> int:
+    return _load().oracle_set_threads(int(n))
+
+
+def lattice(Q: int):
+    """Direction table, weights, opposite index, moment matrix M, M^-1 and row orders."""
+    lib = _load()
+    e = np.zeros((Q, 3), dtype=np.int32)
+    w = np.zeros(Q)
+    opp = np.zeros(Q, dtype=np.int32)
+    M = np.zeros((Q, Q))
+    Minv = np.zeros((Q, Q))
+    order = np.zeros(Q, dtype=np.int32)
+    ip = C.POINTER(C.c_int)
+    rc = lib.oracle_lattice(Q, e.ctypes.data_as(ip), _dp(w), opp.ctypes.data_as(ip), _dp(M), _dp(Minv),
+                            order.ctypes.data_as(ip))
+    if rc:
+        raise ValueError(f"unsupported stencil D3Q{Q}")
+    return e, w, opp, M, Minv, order
+
+
+class Oracle:
+    """Host-side twin of the acm_* call list."""
+
+    def __init__(self, nx, ny, nz, stencil_phase=15, stencil_hydro=19, rho_H=1.0, rho_L=1e-3, sigma=1e-4, xi=5.0,
+                 M=0.02, nu_H=1 / 60, nu_L=1 / 60, gravity=(0.0, 0.0, 0.0), wall_flags=0):
+        self._lib = _load()
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.Qh, self.Qg = int(stencil_phase), int(stencil_hydro)
+        self.N = self.nx * self.ny * self.nz
+        self.shape = (self.nz, self.ny, self.nx)
+        g = (C.c_double * 3)(*[float(v) for v in gravity])
+        h = C.c_void_p()
+        rc = self._lib.oracle_create(C.byref(h), self.nx, self.ny, self.nz, self.Qh, self.Qg, rho_H, rho_L, sigma, xi,
+                                     M, nu_H, nu_L, g, int(wall_flags))
+        if rc:
+            raise ValueError(f"oracle_create failed with code {rc}")
+        self._h = h
+
+    @classmethod
+    def from_params(cls, p):
+        return cls(p.nx, p.ny, p.nz, p.stencil_phase, p.stencil_hydro, p.rho_H, p.rho_L, p.sigma, p.xi, p.M,
+                   p.nu_H, p.nu_L, p.gravity, p.wall_flags)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.oracle_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def init(self, phi, u):
+        phi = np.ascontiguousarray(phi, dtype=np.float64).reshape(self.shape)
+        u = np.ascontiguousarray(u, dtype=np.float64).reshape((3,) + self.shape)
+        rc = self._lib.oracle_init(self._h, _dp(phi), _dp(u))
+        assert rc == 0, rc
+
+    def step(self, n=1):
+        rc = self._lib.oracle_step(self._h, int(n))
+        if rc:
+            raise RuntimeError(f"oracle_step failed with code {rc}")
+
+    def fields(self, want_p=True):
+        phi = np.empty(self.shape)
+        u = np.empty((3,) + self.shape)
+        p = np.empty(self.shape) if want_p else None
+        self._lib.oracle_fields(self._h, _dp(phi), _dp(u), _dp(p))
+        return phi, u, p
+
+    def phi_mass(self):
+        t = C.c_double()
+        rc = self._lib.oracle_phi_mass(self._h, C.byref(t))
+        if rc:
+            raise FloatingPointError("sum(phi) is not finite")
+        return t.value
+
+    def get_pdfs(self):
+        h = np.empty((self.Qh,) + self.shape)
+        g = np.empty((self.Qg,) + self.shape)
+        self._lib.oracle_get_pdfs(self._h, _dp(h), _dp(g))
+        return h, g
+
+    def set_pdfs(self, h=None, g=None):
+        h = None if h is None else np.ascontiguousarray(h, dtype=np.float64).reshape((self.Qh,) + self.shape)
+        g = None if g is None else np.ascontiguousarray(g, dtype=np.float64).reshape((self.Qg,) + self.shape)
+        self._lib.oracle_set_pdfs(self._h, _dp(h), _dp(g))
+
+    def fd(self, field, hydro_stencil=False):
+        field = np.ascontiguousarray(field, dtype=np.float64).reshape(self.shape)
+        grad = np.empty((3,) + self.shape)
+        lap = np.empty(self.shape)
+        self._lib.oracle_fd(self._h, int(hydro_stencil), _dp(field), _dp(grad), _dp(lap))
+        return grad, lap
