@@ -1,0 +1,134 @@
+/*
+ * acm.h -- C ABI of libacm: the per-time-step coupled lattice-Boltzmann update of the
+ * conservative Allen-Cahn model (ACM) for immiscible fluids at high density ratio,
+ * arXiv 2012.06144 (PAPER.md "P:<line>"), as hand-written CUDA kernels for sm_100a (B200).
+ *
+ * What one time step computes (Algorithm 2; equations of section 3):
+ *   1. phase-field LB step: stream-pull the populations h_i, phi = sum_i h_i (eq. 7),
+ *      isotropic finite-difference grad phi (eq. 23), interface normal n, Allen-Cahn forcing
+ *      (eq. 5), MRT collision (eq. 4), store h and phi               -- ONE kernel;
+ *   2. hydrodynamic LB step: velocity-based populations g_i, rho(phi) (eq. 8),
+ *      chemical potential (eq. 17), surface-tension, pressure, viscous and body force
+ *      (eqs. 13-18, 30), tau(phi) (eqs. 20-21), velocity (eq. 22), MRT collision
+ *      (eqs. 10-12, 25), streaming, store g and u                          -- ONE kernel.
+ * Readings of the paper where it is silent or garbled are listed in DESIGN.md.
+ *
+ * Conventions
+ *   - All field arrays are structure-of-arrays with x fastest: element (q, x, y, z) of a
+ *     population array lives at ((q*nz + z)*ny + y)*nx + x; u is component-major (3 planes).
+ *   - Element type of every `void*` field pointer follows `precision` of acm_create
+ *     (ACM_F64: double, ACM_F32: float).
+ *   - Direction order ("canonical order") of the population arrays exchanged through
+ *     acm_get_pdfs: rest; (+x,-x,+y,-y,+z,-z); the 12 edge directions
+ *     (+1,+1,0)(-1,-1,0)(+1,-1,0)(-1,+1,0)(+1,0,+1)(-1,0,-1)(+1,0,-1)(-1,0,+1)
+ *     (0,+1,+1)(0,-1,-1)(0,+1,-1)(0,-1,+1); the 8 corner directions
+ *     (+1,+1,+1)(-1,-1,-1)(+1,+1,-1)(-1,-1,+1)(+1,-1,+1)(-1,+1,-1)(-1,+1,+1)(+1,-1,-1).
+ *     D3Q15 = rest+axis+corner, D3Q19 = rest+axis+edge, D3Q27 = all.
+ *   - Ownership: the CALLER owns all device memory.  The library never allocates device
+ *     memory; acm_create carves the caller's workspace.  The context (host memory) is
+ *     freed by acm_destroy only.
+ *   - Pointers marked [device] must be device pointers valid on the current CUDA device,
+ *     pointers marked [host] are ordinary host pointers (pinned memory makes the copies
+ *     asynchronous but is not required).
+ *   - Every call returns an ACM_* code and never throws; acm_last_error() describes the
+ *     last failure of the calling thread.  CUDA errors are sticky: once a launch failed,
+ *     every later call on the context returns ACM_ECUDA.
+ *   - All work is issued on the stream given to acm_create; calls are asynchronous with
+ *     respect to the host unless stated otherwise.
+ */
+#ifndef ACM_H_
+#define ACM_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct acm_ctx acm_ctx; /* opaque; owns no device memory */
+
+enum { ACM_OK = 0, ACM_EINVAL = 1, ACM_ESTATE = 2, ACM_ECUDA = 3, ACM_EUNSTABLE = 4 };
+enum { ACM_D3Q15 = 15, ACM_D3Q19 = 19, ACM_D3Q27 = 27 };
+/* set: half-way bounce-back no-slip walls on both faces of that axis; clear: periodic */
+enum { ACM_WALL_X = 1, ACM_WALL_Y = 2, ACM_WALL_Z = 4 };
+enum { ACM_F64 = 0, ACM_F32 = 1 };
+
+/* Bytes of device workspace acm_create needs for this configuration (two grids of h and g,
+ * two phi buffers, u, a 5N staging area for the *_host calls and reduction scratch), or 0 if
+ * the configuration is invalid. */
+size_t acm_workspace_bytes(int nx, int ny, int nz, int stencil_phase, int stencil_hydro, int precision);
+
+/* Creates a context.  Parameters follow the paper's statement of the problem:
+ *   nx,ny,nz        grid size in cells (each >= 1; nx*ny*nz < 2^31)
+ *   stencil_phase   lattice of h: ACM_D3Q15 | ACM_D3Q19 | ACM_D3Q27
+ *   stencil_hydro   lattice of g: ACM_D3Q19 | ACM_D3Q27 (ACM_D3Q15 also accepted)
+ *   rho_H, rho_L    densities of the heavy / light phase, rho_H >= rho_L > 0   (eq. 8)
+ *   sigma           surface tension >= 0; beta = 12 sigma/xi, kappa = 3 sigma xi/2
+ *   xi              interface thickness > 0
+ *   M               mobility > 0; tau_phi = M/c_s^2 (eq. 2), first-order moments of h relax
+ *                   with 1/(tau_phi + 1/2)
+ *   nu_H, nu_L      kinematic viscosities > 0; tau = nu/c_s^2 (eq. 19) interpolated linearly
+ *                   in phi (eq. 20), s_nu = 1/(tau + 1/2) (eq. 21)
+ *   gravity[3]      [host] acceleration g of the body force F_b = rho g (eq. 30); NULL = 0
+ *   wall_flags      OR of ACM_WALL_*
+ *   precision       ACM_F64 (the paper's precision) or ACM_F32
+ *   workspace       [device] >= acm_workspace_bytes() bytes, 256-byte aligned, caller-owned,
+ *                   must outlive the context
+ *   cuda_stream     a cudaStream_t (NULL = legacy default stream)
+ * Errors: ACM_EINVAL for any violated constraint above (and *out = NULL). */
+int acm_create(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int stencil_hydro,
+               double rho_H, double rho_L, double sigma, double xi, double M, double nu_H, double nu_L,
+               const double gravity[3], unsigned wall_flags, int precision,
+               void* workspace, void* cuda_stream);
+
+/* Equilibrium initialiser ("Initialisation of all fields", Alg. 2 line 1):
+ * phi-field <- phi, u-field <- u, h_i <- phi Gamma_i(u) (eq. 6), g_i <- Gamma_i(u) - w_i
+ * (eq. 12 with p* = 0).  phi: [device] N values; u: [device] 3N values, component-major. */
+int acm_init(acm_ctx*, const void* phi, const void* u);
+
+/* Advances n >= 0 time steps (phase-field kernel, then hydrodynamic kernel, per step).
+ * Asynchronous.  ACM_ESTATE before acm_init. */
+int acm_step(acm_ctx*, int n);
+
+/* Copies out the macroscopic fields of the current time level: phi (N), u (3N, as stored by
+ * the last hydrodynamic step, eq. 22) and the pressure p = p* rho(phi) c_s^2 with
+ * p* = sum_i g_i (eq. 15).  [device] pointers; any may be NULL = skipped. */
+int acm_fields(acm_ctx*, void* phi, void* u, void* p);
+
+/* Total phase-field mass sum_x phi(x) (eq. 7 summed over the grid), accumulated in fp64 by a
+ * deterministic two-pass block reduction.  Synchronises the stream.  total_host: [host].
+ * ACM_EUNSTABLE if the sum is not finite. */
+int acm_phi_mass(acm_ctx*, double* total_host);
+
+/* Parity/debug export of the populations in canonical direction order and in the storage
+ * convention of the paper's two LB steps: h = post-collision values at their cell (they are
+ * pulled by the next phase step), g = streamed values (collide-stream-push).
+ * h: [device] Q_h*N, g: [device] Q_g*N; either may be NULL. */
+int acm_get_pdfs(acm_ctx*, void* h, void* g);
+
+/* Overwrites the populations (same layout and convention as acm_get_pdfs); lets a test
+ * plant an arbitrary non-equilibrium state.  Either pointer may be NULL. */
+int acm_set_pdfs(acm_ctx*, const void* h, const void* g);
+
+/* End-to-end convenience with HOST buffers: copies phi (N) and u (3N) to the device,
+ * acm_init, acm_step(n), then copies phi/u/p of the final state back (NULL = skipped) and
+ * synchronises the stream.  Equivalent to the calls above plus the transfers. */
+int acm_run_host(acm_ctx*, const void* phi_host, const void* u_host, int n,
+                 void* phi_out_host, void* u_out_host, void* p_out_host);
+
+/* Launch geometry of the two LB kernels (threads per block along x, y, z; product <= 1024).
+ * Optional; the defaults are tuned for B200. */
+int acm_set_block(acm_ctx*, int bx, int by, int bz);
+
+/* Number of kernels this context has launched so far (bench.py's gpu_launches). */
+long long acm_launch_count(const acm_ctx*);
+
+void acm_destroy(acm_ctx*);
+
+/* Thread-local description of the last error; never NULL. */
+const char* acm_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ACM_H_ */

@@ -1,0 +1,169 @@
+"""Thin Python binding of libacm.so (include/acm.h): argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the path runs in the
+library's CUDA kernels.  There is no fallback: a missing library or a missing GPU raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+from . import build as _build
+
+ACM_OK, ACM_EINVAL, ACM_ESTATE, ACM_ECUDA, ACM_EUNSTABLE = 0, 1, 2, 3, 4
+ACM_F64, ACM_F32 = 0, 1
+ACM_WALL_X, ACM_WALL_Y, ACM_WALL_Z = 1, 2, 4
+
+EXPORTS = ["acm_workspace_bytes", "acm_create", "acm_init", "acm_step", "acm_fields", "acm_phi_mass", "acm_get_pdfs",
+           "acm_set_pdfs", "acm_run_host", "acm_set_block", "acm_launch_count", "acm_destroy", "acm_last_error"]
+
+_lib = None
+
+
+class AcmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libacm error {code}: {msg}")
+        self.code = code
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load(build_if_missing: bool = True):
+    """Loads libacm.so (building it with nvcc if it is absent and nvcc exists)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        if not build_if_missing:
+            raise RuntimeError(f"{path} is missing: run `python -m paper_2012_06144_b200.build`")
+        _build.build_lib()
+    lib = C.CDLL(path)
+    vp, dbl, i32 = C.c_void_p, C.c_double, C.c_int
+    lib.acm_workspace_bytes.restype = C.c_size_t
+    lib.acm_workspace_bytes.argtypes = [i32] * 6
+    lib.acm_create.argtypes = [C.POINTER(vp)] + [i32] * 5 + [dbl] * 7 + [C.POINTER(dbl), C.c_uint, i32, vp, vp]
+    lib.acm_init.argtypes = [vp, vp, vp]
+    lib.acm_step.argtypes = [vp, i32]
+    lib.acm_fields.argtypes = [vp, vp, vp, vp]
+    lib.acm_phi_mass.argtypes = [vp, C.POINTER(dbl)]
+    lib.acm_get_pdfs.argtypes = [vp, vp, vp]
+    lib.acm_set_pdfs.argtypes = [vp, vp, vp]
+    lib.acm_run_host.argtypes = [vp, vp, vp, i32, vp, vp, vp]
+    lib.acm_set_block.argtypes = [vp, i32, i32, i32]
+    lib.acm_launch_count.argtypes = [vp]
+    lib.acm_launch_count.restype = C.c_longlong
+    lib.acm_destroy.argtypes = [vp]
+    lib.acm_destroy.restype = None
+    lib.acm_last_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(lib, rc):
+    if rc != ACM_OK:
+        raise AcmError(rc, lib.acm_last_error().decode())
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+class ACM:
+    """One simulation context: acm_create / acm_init / acm_step / acm_fields / acm_phi_mass."""
+
+    def __init__(self, nx, ny, nz, stencil_phase=15, stencil_hydro=19, rho_H=1.0, rho_L=1e-3, sigma=1e-4, xi=5.0,
+                 M=0.02, nu_H=1 / 60, nu_L=1 / 60, gravity=(0.0, 0.0, 0.0), wall_flags=0, precision="f64",
+                 device="cuda:0", stream=None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2012_06144_b200 needs a CUDA device (no CPU fallback)")
+        self._lib = load()
+        self.device = torch.device(device)
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.Qh, self.Qg = int(stencil_phase), int(stencil_hydro)
+        self.N = self.nx * self.ny * self.nz
+        self.shape = (self.nz, self.ny, self.nx)
+        self.precision = {"f64": ACM_F64, "f32": ACM_F32}[precision]
+        self.dtype = torch.float64 if precision == "f64" else torch.float32
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        nbytes = self._lib.acm_workspace_bytes(self.nx, self.ny, self.nz, self.Qh, self.Qg, self.precision)
+        if nbytes == 0:
+            raise AcmError(ACM_EINVAL, "invalid grid size / stencil / precision")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = (self.workspace.data_ptr() + 255) & ~255
+        g = (C.c_double * 3)(*[float(v) for v in gravity])
+        h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            rc = self._lib.acm_create(C.byref(h), self.nx, self.ny, self.nz, self.Qh, self.Qg, rho_H, rho_L, sigma, xi,
+                                      M, nu_H, nu_L, g, int(wall_flags), self.precision, C.c_void_p(base),
+                                      C.c_void_p(self.stream.cuda_stream))
+        _check(self._lib, rc)
+        self._h = h
+
+    @classmethod
+    def from_params(cls, p, **kw):
+        return cls(p.nx, p.ny, p.nz, p.stencil_phase, p.stencil_hydro, p.rho_H, p.rho_L, p.sigma, p.xi, p.M, p.nu_H,
+                   p.nu_L, p.gravity, p.wall_flags, **kw)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.acm_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def _call(self, fn, *args):
+        with torch.cuda.device(self.device):
+            _check(self._lib, fn(self._h, *args))
+
+    def _dev(self, t, shape):
+        assert t.is_cuda and t.dtype == self.dtype and t.is_contiguous() and tuple(t.shape) == tuple(shape), \
+            (t.device, t.dtype, t.shape, shape)
+        return _ptr(t)
+
+    def set_block(self, bx, by=1, bz=1):
+        self._call(self._lib.acm_set_block, int(bx), int(by), int(bz))
+
+    def init(self, phi, u):
+        self._call(self._lib.acm_init, self._dev(phi, self.shape), self._dev(u, (3,) + self.shape))
+
+    def step(self, n=1):
+        self._call(self._lib.acm_step, int(n))
+
+    def fields(self, want_p=True):
+        phi = torch.empty(self.shape, dtype=self.dtype, device=self.device)
+        u = torch.empty((3,) + self.shape, dtype=self.dtype, device=self.device)
+        p = torch.empty(self.shape, dtype=self.dtype, device=self.device) if want_p else None
+        self._call(self._lib.acm_fields, _ptr(phi), _ptr(u), _ptr(p))
+        return phi, u, p
+
+    def phi_mass(self):
+        t = C.c_double()
+        self._call(self._lib.acm_phi_mass, C.byref(t))
+        return t.value
+
+    def get_pdfs(self):
+        h = torch.empty((self.Qh,) + self.shape, dtype=self.dtype, device=self.device)
+        g = torch.empty((self.Qg,) + self.shape, dtype=self.dtype, device=self.device)
+        self._call(self._lib.acm_get_pdfs, _ptr(h), _ptr(g))
+        return h, g
+
+    def set_pdfs(self, h=None, g=None):
+        hp = None if h is None else self._dev(h, (self.Qh,) + self.shape)
+        gp = None if g is None else self._dev(g, (self.Qg,) + self.shape)
+        self._call(self._lib.acm_set_pdfs, hp, gp)
+
+    def run_host(self, phi_host, u_host, n, phi_out=None, u_out=None, p_out=None):
+        """Host buffers in (CPU tensors, ideally pinned), host buffers out; transfers inside."""
+        for t in (phi_host, u_host, phi_out, u_out, p_out):
+            assert t is None or (not t.is_cuda and t.dtype == self.dtype and t.is_contiguous())
+        self._call(self._lib.acm_run_host, _ptr(phi_host), _ptr(u_host), int(n), _ptr(phi_out), _ptr(u_out), _ptr(p_out))
+
+    @property
+    def launch_count(self):
+        return int(self._lib.acm_launch_count(self._h))

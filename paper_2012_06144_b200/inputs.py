@@ -121,10 +121,28 @@ def bubble_set(p: Params, count: int, r_min: float, r_max: float, seed: int = SE
 
 
 def bubbles_phi(p: Params, centres, radii):
-    """phi = 1/2 + 1/2 tanh(2 min_b(d_b - R_b)/xi): light bubbles in heavy liquid."""
+    """phi = 1/2 + 1/2 tanh(2 min_b(d_b - R_b)/xi): light bubbles in heavy liquid.
+
+    Each bubble only touches the cells within R + 12 xi of its centre: beyond that
+    tanh(2 (d-R)/xi) = tanh(24) rounds to exactly 1.0 in fp64, which is also what the
+    untouched cells get (min over an empty set = +inf), so the result equals the full min."""
     dmin = np.full(p.shape, np.inf)
+    n = (p.nx, p.ny, p.nz)
     for c, R in zip(centres, radii):
-        np.minimum(dmin, _distance(p, c) - R, out=dmin)
+        reach = R + 12.0 * p.xi
+        idx, dist2 = [], []
+        for a in range(3):
+            lo, hi = int(np.floor(c[a] - reach)) - 1, int(np.ceil(c[a] + reach)) + 1
+            if hi - lo >= n[a]:
+                lo, hi = 0, n[a]
+            ia = np.arange(lo, hi) % n[a]
+            d = np.abs(ia + 0.5 - c[a])
+            d = np.minimum(d, n[a] - d)
+            idx.append(ia)
+            dist2.append(d * d)
+        sub = np.ix_(idx[2], idx[1], idx[0])
+        d = np.sqrt(dist2[2][:, None, None] + dist2[1][None, :, None] + dist2[0][None, None, :]) - R
+        dmin[sub] = np.minimum(dmin[sub], d)
     return 0.5 + 0.5 * np.tanh(2.0 * dmin / p.xi)
 
 

@@ -1,0 +1,58 @@
+"""The C-ABI library builds, loads and exports every symbol include/acm.h declares (no GPU needed)."""
+import ctypes
+import os
+import re
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "acm.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(acm_[a-z_]+)\s*\(", src)))
+
+
+def test_header_symbols_exported():
+    from paper_2012_06144_b200 import binding, build
+    path = build.build_lib()
+    lib = ctypes.CDLL(path)
+    names = _declared()
+    assert len(names) >= 12
+    for n in names:
+        assert hasattr(lib, n), n
+    assert sorted(binding.EXPORTS) == names
+
+
+def test_workspace_bytes_and_argument_checks():
+    """Host-only entry points: size arithmetic and acm_create argument validation (no kernel runs)."""
+    from paper_2012_06144_b200 import binding
+    lib = binding.load()
+    N = 32 ** 3
+    b = lib.acm_workspace_bytes(32, 32, 32, 15, 19, 0)
+    payload = (2 * (15 + 19) + 2 + 3 + 5) * N * 8
+    assert payload <= b <= payload + 16 * 256 + 8192
+    assert lib.acm_workspace_bytes(32, 32, 32, 15, 19, 1) < b
+    assert lib.acm_workspace_bytes(0, 32, 32, 15, 19, 0) == 0
+    assert lib.acm_workspace_bytes(32, 32, 32, 13, 19, 0) == 0
+    assert lib.acm_workspace_bytes(2048, 2048, 2048, 15, 19, 0) == 0      # >= 2^31 cells
+    h = ctypes.c_void_p()
+    g = (ctypes.c_double * 3)(0, 0, 0)
+    fake_ws = ctypes.c_void_p(256 * 1000)
+
+    def create(**kw):
+        a = dict(nx=8, ny=8, nz=8, qh=15, qg=19, rho_H=1.0, rho_L=1e-3, sigma=1e-4, xi=5.0, M=0.02, nu_H=1 / 60,
+                 nu_L=1 / 60, walls=0, prec=0, ws=fake_ws)
+        a.update(kw)
+        return lib.acm_create(ctypes.byref(h), a["nx"], a["ny"], a["nz"], a["qh"], a["qg"], a["rho_H"], a["rho_L"],
+                              a["sigma"], a["xi"], a["M"], a["nu_H"], a["nu_L"], g, a["walls"], a["prec"], a["ws"], None)
+
+    for bad in (dict(nx=0), dict(qh=9), dict(rho_L=0.0), dict(rho_H=1e-4), dict(xi=0.0), dict(M=0.0), dict(nu_L=-1.0),
+                dict(walls=8), dict(prec=2), dict(ws=None), dict(ws=ctypes.c_void_p(8)), dict(sigma=-1.0)):
+        assert create(**bad) == binding.ACM_EINVAL, bad
+        assert h.value is None
+        assert len(lib.acm_last_error()) > 0
+    assert create() == binding.ACM_OK and h.value
+    assert lib.acm_step(h, 1) == binding.ACM_ESTATE          # before acm_init
+    assert lib.acm_step(h, -1) == binding.ACM_EINVAL
+    assert lib.acm_launch_count(h) == 0
+    lib.acm_destroy(h)
