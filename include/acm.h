@@ -120,6 +120,14 @@ int acm_run_host(acm_ctx*, const void* phi_host, const void* u_host, int n,
  * Optional; the defaults are tuned for B200. */
 int acm_set_block(acm_ctx*, int bx, int by, int bz);
 
+/* Per-kernel device timing for the roofline report.  acm_profile(ctx, 1) makes every later
+ * acm_step record CUDA events on the stream around each of its two kernels (and drops earlier
+ * records); acm_profile(ctx, 0) switches that off.  acm_profile_read synchronises the stream,
+ * returns the summed durations in milliseconds of the phase-field and the hydrodynamic kernel
+ * and the number of steps they cover, and clears the records.  Pointers are [host], may be NULL. */
+int acm_profile(acm_ctx*, int enable);
+int acm_profile_read(acm_ctx*, double* phase_ms, double* hydro_ms, long long* steps);
+
 /* Number of kernels this context has launched so far (bench.py's gpu_launches). */
 long long acm_launch_count(const acm_ctx*);
 

@@ -17,7 +17,7 @@ ACM_F64, ACM_F32 = 0, 1
 ACM_WALL_X, ACM_WALL_Y, ACM_WALL_Z = 1, 2, 4
 
 EXPORTS = ["acm_workspace_bytes", "acm_create", "acm_init", "acm_step", "acm_fields", "acm_phi_mass", "acm_get_pdfs",
-           "acm_set_pdfs", "acm_run_host", "acm_set_block", "acm_launch_count", "acm_destroy", "acm_last_error"]
+           "acm_set_pdfs", "acm_run_host", "acm_set_block", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
 
 _lib = None
 
@@ -55,6 +55,8 @@ def load(build_if_missing: bool = True):
     lib.acm_set_pdfs.argtypes = [vp, vp, vp]
     lib.acm_run_host.argtypes = [vp, vp, vp, i32, vp, vp, vp]
     lib.acm_set_block.argtypes = [vp, i32, i32, i32]
+    lib.acm_profile.argtypes = [vp, i32]
+    lib.acm_profile_read.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(C.c_longlong)]
     lib.acm_launch_count.argtypes = [vp]
     lib.acm_launch_count.restype = C.c_longlong
     lib.acm_destroy.argtypes = [vp]
@@ -163,6 +165,15 @@ class ACM:
         for t in (phi_host, u_host, phi_out, u_out, p_out):
             assert t is None or (not t.is_cuda and t.dtype == self.dtype and t.is_contiguous())
         self._call(self._lib.acm_run_host, _ptr(phi_host), _ptr(u_host), int(n), _ptr(phi_out), _ptr(u_out), _ptr(p_out))
+
+    def profile(self, enable=True):
+        self._call(self._lib.acm_profile, int(bool(enable)))
+
+    def profile_read(self):
+        """(phase_ms, hydro_ms, steps) summed over the acm_step calls since profile(True)."""
+        a, b, n = C.c_double(), C.c_double(), C.c_longlong()
+        self._call(self._lib.acm_profile_read, C.byref(a), C.byref(b), C.byref(n))
+        return a.value, b.value, n.value
 
     @property
     def launch_count(self):

@@ -17,6 +17,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "../../include/acm.h"
 #include "lattice.cuh"
@@ -428,6 +429,10 @@ struct acm_ctx {
     int sticky;                 // ACM_OK or ACM_ECUDA
     dim3 block;
     long long launches;
+    // optional per-kernel timing (acm_profile): events recorded around every LB kernel
+    bool profiling;
+    std::vector<cudaEvent_t> ev;     // per acm_step call: e0 [phase] e1 [hydro] e2 [phase] ...
+    std::vector<int> ev_calls;       // number of steps of each recorded acm_step call
 };
 
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
@@ -560,15 +565,27 @@ static int init_t(acm_ctx* c, const void* phi, const void* u)
     return rc;
 }
 
+static void prof_mark(acm_ctx* c)
+{
+    if (!c->profiling) return;
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) return;
+    cudaEventRecord(e, c->stream);
+    c->ev.push_back(e);
+}
+
 template <typename T>
 static int step_t(acm_ctx* c, int n)
 {
+    if (c->profiling && n > 0) { c->ev_calls.push_back(n); prof_mark(c); }
     for (int t = 0; t < n; ++t) {
         int rc = ACM_OK;
         ACM_DISPATCH_Q(c->Qh, QH, rc = launch_phase<T, QH>(c));
         if (rc) return rc;
+        prof_mark(c);
         ACM_DISPATCH_Q(c->Qg, QG, rc = launch_hydro<T, QG>(c));
         if (rc) return rc;
+        prof_mark(c);
     }
     return ACM_OK;
 }
@@ -648,11 +665,58 @@ int acm_create(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int ste
     c->sticky = ACM_OK;
     c->block = dim3(128, 1, 1);
     c->launches = 0;
+    c->profiling = false;
     *out = c;
     return ACM_OK;
 }
 
-void acm_destroy(acm_ctx* c) { delete c; }
+static void prof_clear(acm_ctx* c)
+{
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    c->ev.clear();
+    c->ev_calls.clear();
+}
+
+void acm_destroy(acm_ctx* c)
+{
+    if (!c) return;
+    prof_clear(c);
+    delete c;
+}
+
+int acm_profile(acm_ctx* c, int enable)
+{
+    ACM_CHECK_CTX(c);
+    prof_clear(c);
+    c->profiling = enable != 0;
+    return ACM_OK;
+}
+
+int acm_profile_read(acm_ctx* c, double* phase_ms, double* hydro_ms, long long* steps)
+{
+    ACM_CHECK_CTX(c);
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) { c->sticky = ACM_ECUDA; return fail(ACM_ECUDA, "acm_profile_read: %s", cudaGetErrorString(e)); }
+    double ph = 0.0, hy = 0.0;
+    long long ns = 0;
+    size_t k = 0;
+    for (int n : c->ev_calls) {
+        if (k + 2 * (size_t)n + 1 > c->ev.size()) break;
+        for (int t = 0; t < n; ++t) {
+            float a = 0.f, b = 0.f;
+            cudaEventElapsedTime(&a, c->ev[k + 2 * t], c->ev[k + 2 * t + 1]);
+            cudaEventElapsedTime(&b, c->ev[k + 2 * t + 1], c->ev[k + 2 * t + 2]);
+            ph += a; hy += b;
+        }
+        ns += n;
+        k += 2 * (size_t)n + 1;
+    }
+    if (phase_ms) *phase_ms = ph;
+    if (hydro_ms) *hydro_ms = hy;
+    if (steps) *steps = ns;
+    prof_clear(c);
+    return ACM_OK;
+}
 
 int acm_set_block(acm_ctx* c, int bx, int by, int bz)
 {

@@ -1,0 +1,219 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (north_star): max|d pdf| <= 1e-13 after 1 step; max|d phi|, |d u| <= 1e-10 after 100
+steps (fp64, lattice units).  All tests need a GPU (-m gpu).
+"""
+import numpy as np
+import pytest
+import torch
+
+from helpers import random_state
+from oracle import Oracle
+from paper_2012_06144_b200 import inputs
+from paper_2012_06144_b200.inputs import Params
+
+pytestmark = pytest.mark.gpu
+
+TOL_PDF_1STEP = 1e-13
+TOL_FIELD_100 = 1e-10
+
+
+def _acm(p, **kw):
+    from paper_2012_06144_b200.binding import ACM
+    return ACM.from_params(p, **kw)
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _run_both(p, phi, u, steps, block=None):
+    o = Oracle.from_params(p)
+    o.init(phi, u)
+    a = _acm(p)
+    if block:
+        a.set_block(*block)
+    a.init(_dev(phi), _dev(u))
+    o.step(steps)
+    a.step(steps)
+    return o, a
+
+
+def _compare_fields(o, a, tol):
+    po, uo, pro = o.fields()
+    pa, ua, pra = a.fields()
+    dphi = np.abs(pa.cpu().numpy() - po).max()
+    du = np.abs(ua.cpu().numpy() - uo).max()
+    dp = np.abs(pra.cpu().numpy() - pro).max()
+    assert dphi <= tol, dphi
+    assert du <= tol, du
+    assert dp <= tol, dp
+    return dphi, du
+
+
+ONE_STEP = [
+    # (nx, ny, nz, Qh, Qg, walls, gravity, block)   -- ragged sizes spanning several blocks
+    (150, 7, 5, 15, 19, 0, (0.0, 0.0, 0.0), (128, 1, 1)),
+    (70, 9, 6, 15, 19, inputs.WALL_Y, (0.0, -1e-5, 0.0), (32, 2, 2)),
+    (37, 6, 11, 27, 27, 0, (1e-5, 0.0, 2e-5), (32, 4, 2)),
+    (33, 5, 4, 19, 27, inputs.WALL_X | inputs.WALL_Z, (0.0, 1e-5, 0.0), (64, 1, 1)),
+    (20, 12, 9, 27, 19, inputs.WALL_X | inputs.WALL_Y | inputs.WALL_Z, (0.0, 0.0, -1e-5), (32, 2, 1)),
+    (16, 8, 8, 15, 15, 0, (0.0, 0.0, 0.0), (16, 4, 4)),
+]
+
+
+@pytest.mark.parametrize("nx,ny,nz,Qh,Qg,walls,grav,block", ONE_STEP)
+def test_one_step_pdf_parity(nx, ny, nz, Qh, Qg, walls, grav, block):
+    """One coupled step from a random non-equilibrium state: every population within 1e-13."""
+    p = Params(nx=nx, ny=ny, nz=nz, stencil_phase=Qh, stencil_hydro=Qg, wall_flags=walls, gravity=grav,
+               rho_H=1.0, rho_L=1e-3, sigma=1e-4, nu_H=0.05, nu_L=1 / 60)
+    phi, u, h, g = random_state(p, seed=11)
+    o = Oracle.from_params(p)
+    o.init(phi, u)
+    o.set_pdfs(h, g)
+    a = _acm(p)
+    a.set_block(*block)
+    a.init(_dev(phi), _dev(u))
+    a.set_pdfs(_dev(h), _dev(g))
+    # set/get round trip is exact (g goes through the lazy-pull scatter/gather)
+    h0, g0 = a.get_pdfs()
+    assert (h0.cpu().numpy() == h).all() and (g0.cpu().numpy() == g).all()
+    o.step(1)
+    a.step(1)
+    ho, go = o.get_pdfs()
+    ha, ga = a.get_pdfs()
+    assert np.abs(ha.cpu().numpy() - ho).max() <= TOL_PDF_1STEP
+    assert np.abs(ga.cpu().numpy() - go).max() <= TOL_PDF_1STEP
+    _compare_fields(o, a, TOL_PDF_1STEP)
+
+
+def test_init_parity():
+    """Equilibrium initialiser: populations equal the oracle's to rounding, fields bitwise."""
+    p = Params(nx=40, ny=6, nz=5, stencil_phase=27, stencil_hydro=19, wall_flags=inputs.WALL_Y)
+    phi, u, _, _ = random_state(p, seed=5)
+    o = Oracle.from_params(p)
+    o.init(phi, u)
+    a = _acm(p)
+    a.init(_dev(phi), _dev(u))
+    ho, go = o.get_pdfs()
+    ha, ga = a.get_pdfs()
+    assert np.abs(ha.cpu().numpy() - ho).max() <= 1e-15
+    assert np.abs(ga.cpu().numpy() - go).max() <= 1e-15
+    pa, ua, _ = a.fields()
+    assert (pa.cpu().numpy() == phi).all() and (ua.cpu().numpy() == u).all()
+
+
+def test_config1_100_steps():
+    """Config 1 (32^3 static droplet): phi, u, p within 1e-10 after 100 steps; sum(phi) conserved."""
+    p, phi, u = inputs.config1()
+    o, a = _run_both(p, phi, u, 100)
+    _compare_fields(o, a, TOL_FIELD_100)
+    m0 = phi.sum()
+    assert abs(a.phi_mass() - m0) / m0 < 1e-12
+    assert abs(a.phi_mass() - o.phi_mass()) / m0 < 1e-13
+
+
+def test_config2_scaled_walls_gravity_100_steps():
+    """Config 2 scaled to 24x48x24 (walls in y, gravity, light bubble near the lower wall)."""
+    p, phi, u = inputs.config2(nx=24, ny=48, nz=24, R=6.0, gy=-1e-6, centre=(12.0, 9.0, 12.0))
+    o, a = _run_both(p, phi, u, 100, block=(32, 2, 2))
+    _compare_fields(o, a, TOL_FIELD_100)
+    m0 = phi.sum()
+    assert abs(a.phi_mass() - m0) / m0 < 1e-12
+
+
+def test_config3_scaled_bubbles_noise_100_steps():
+    """Config 3 scaled to 40^3: seeded bubbles + velocity noise."""
+    p, phi, u = inputs.scaled_config3(40)
+    o, a = _run_both(p, phi, u, 100)
+    _compare_fields(o, a, TOL_FIELD_100)
+
+
+def test_config5_scaled_q27_50_steps():
+    """Config 5 (D3Q27 + D3Q27) scaled to 32^3."""
+    p, phi, u = inputs.scaled_config3(32, stencil_phase=27, stencil_hydro=27)
+    o, a = _run_both(p, phi, u, 50)
+    _compare_fields(o, a, TOL_FIELD_100)
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 1), (2, 1, 3), (1, 5, 1), (3, 2, 2)])
+def test_degenerate_grids(shape):
+    """Tiny grids where a cell is its own periodic neighbour."""
+    nx, ny, nz = shape
+    p = Params(nx=nx, ny=ny, nz=nz, stencil_phase=27, stencil_hydro=27)
+    phi, u, h, g = random_state(p, seed=2)
+    o = Oracle.from_params(p)
+    o.init(phi, u)
+    o.set_pdfs(h, g)
+    a = _acm(p)
+    a.init(_dev(phi), _dev(u))
+    a.set_pdfs(_dev(h), _dev(g))
+    o.step(3)
+    a.step(3)
+    ho, go = o.get_pdfs()
+    ha, ga = a.get_pdfs()
+    assert np.abs(ha.cpu().numpy() - ho).max() <= 1e-12
+    assert np.abs(ga.cpu().numpy() - go).max() <= 1e-12
+
+
+def test_step_zero_and_state_errors():
+    from paper_2012_06144_b200 import binding
+    p, phi, u = inputs.config1(n=8, R=2.0)
+    a = _acm(p)
+    with pytest.raises(binding.AcmError) as e:
+        a.step(1)
+    assert e.value.code == binding.ACM_ESTATE
+    a.init(_dev(phi), _dev(u))
+    a.step(0)
+    pa, ua, _ = a.fields()
+    assert (pa.cpu().numpy() == phi).all()
+    with pytest.raises(binding.AcmError) as e:
+        a.step(-1)
+    assert e.value.code == binding.ACM_EINVAL
+    assert a.launch_count > 0
+
+
+def test_uniform_state_exact():
+    """north_star invariant on the CUDA path: uniform phi at rest stays bitwise uniform, u = 0."""
+    p = Params(nx=64, ny=6, nz=5)
+    a = _acm(p)
+    a.init(_dev(np.full(p.shape, 0.3)), _dev(inputs.zeros_u(p)))
+    a.step(30)
+    pa, ua, _ = a.fields()
+    pa = pa.cpu().numpy()
+    assert (pa == pa.flat[0]).all() and abs(pa.flat[0] - 0.3) < 1e-13
+    assert (ua.cpu().numpy() == 0).all()
+
+
+def test_run_host_matches_device_calls():
+    """acm_run_host (host buffers, transfers inside) == acm_init + acm_step + acm_fields."""
+    p, phi, u = inputs.scaled_config3(24)
+    a = _acm(p)
+    a.init(_dev(phi), _dev(u))
+    a.step(7)
+    pa, ua, pra = a.fields()
+    b = _acm(p)
+    ph = torch.from_numpy(phi).pin_memory()
+    uh = torch.from_numpy(u).pin_memory()
+    po, uo, pro = torch.empty_like(ph).pin_memory(), torch.empty_like(uh).pin_memory(), torch.empty_like(ph).pin_memory()
+    b.run_host(ph, uh, 7, po, uo, pro)
+    assert (po == pa.cpu()).all() and (uo == ua.cpu()).all() and (pro == pra.cpu()).all()
+
+
+def test_laplace_law_gpu():
+    """Config 1 run for 10 000 steps on the GPU: dp = 2 sigma/R within 3 % and equal to the oracle's
+    stored trajectory (tests/golden/laplace_config1.txt, written by the oracle only)."""
+    import os
+    p, phi, u = inputs.config1()
+    a = _acm(p)
+    a.init(_dev(phi), _dev(u))
+    m0 = a.phi_mass()
+    a.step(10000)
+    _, _, pr = a.fields()
+    c = p.nx // 2
+    ratio = float(pr[c, c, c] - pr[0, 0, 0]) / (2 * p.sigma / 8.0)
+    assert abs(ratio - 1.0) < 0.03
+    assert abs(a.phi_mass() - m0) / m0 < 1e-12
+    golden = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "laplace_config1.txt")
+    rows = {int(l.split()[0]): float(l.split()[1]) for l in open(golden) if not l.startswith("#")}
+    assert abs(ratio - rows[10000]) < 1e-6
