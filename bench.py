@@ -252,13 +252,13 @@ def run_acm(args, rank, local_rank, world):
         dom_bytes = (b_hydro if dom == "hydro_kernel" else b_phase) * N
         achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
         step_gbs = (b_phase + b_hydro) * N * K / (ms * 1e-3) / 1e9
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        traffic = None      # DRAM bytes per launch of that kernel from the committed ncu --set full capture
+        tpath = os.path.join(ROOT, "profiles", "traffic.csv")
         if os.path.exists(tpath):
-            try:
-                traffic = json.load(open(tpath)).get(f"{dom}:{args.config}:{precision}")
-            except Exception:
-                traffic = None
+            import csv
+            for row in csv.DictReader(open(tpath)):
+                if (row["kernel"], row["config"], row["precision"]) == (dom, str(args.config), precision):
+                    traffic = float(row["dram_bytes_per_launch"])
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

@@ -29,7 +29,8 @@ class AcmError(RuntimeError):
 
 
 def lib_path() -> str:
-    return _build.LIB
+    """In-tree libacm.so, or the build named by $ACM_LIB (kernel tuning experiments)."""
+    return os.environ.get("ACM_LIB") or _build.LIB
 
 
 def load(build_if_missing: bool = True):

@@ -76,9 +76,45 @@ struct Nbr {
     }
 };
 
-// streaming loads/stores: every population is read once and written once per step
-template <typename T> __device__ __forceinline__ T ld_stream(const T* p) { return __ldcs(p); }
-template <typename T> __device__ __forceinline__ void st_stream(T* p, T v) { __stcs(p, v); }
+// tuning knobs (defaults = the measured best on B200)
+#ifndef ACM_LD
+#define ACM_LD 2
+#endif
+#ifndef ACM_ST
+#define ACM_ST 2
+#endif
+#ifndef ACM_PHASE_MINB
+#define ACM_PHASE_MINB 1
+#endif
+#ifndef ACM_HYDRO_MINB
+#define ACM_HYDRO_MINB 1
+#endif
+#ifndef ACM_MAXT
+#define ACM_MAXT 256
+#endif
+
+// population loads/stores.  Measured on B200 (profiles/r1_variants.md): plain ld/st beat the
+// streaming hints (__ldcs/__stcs) by 5 % on the whole step, so plain is the default.
+template <typename T> __device__ __forceinline__ T ld_stream(const T* p)
+{
+#if ACM_LD == 0
+    return __ldcs(p);
+#elif ACM_LD == 1
+    return __ldg(p);
+#else
+    return *p;
+#endif
+}
+template <typename T> __device__ __forceinline__ void st_stream(T* p, T v)
+{
+#if ACM_ST == 0
+    __stcs(p, v);
+#elif ACM_ST == 1
+    __stcg(p, v);
+#else
+    *p = v;
+#endif
+}
 
 // Pull the Q populations arriving at this cell: f_i(x) <- F_i(x - e_i), or F_ibar(x) if x - e_i
 // lies beyond a wall (half-way bounce-back inside the streaming step).
@@ -145,7 +181,7 @@ struct PhaseArgs {
 };
 
 template <typename T, int Q, bool WALLS>
-__global__ void __launch_bounds__(256) phase_kernel(const PhaseArgs<T> a)
+__global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const PhaseArgs<T> a)
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -210,7 +246,7 @@ struct HydroArgs {
 };
 
 template <typename T, int Q, bool WALLS>
-__global__ void __launch_bounds__(256) hydro_kernel(const HydroArgs<T> a)
+__global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const HydroArgs<T> a)
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
