@@ -174,20 +174,17 @@ def workload_name_only(config):
 
 def run_acm(args, rank, local_rank, world):
     import torch
-    import torch.distributed as dist
+    from paper_2012_06144_b200 import replicas
     from paper_2012_06144_b200.binding import ACM
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+    replicas.init("nccl", dev)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize(dev)
+        replicas.barrier(dev)
 
     K, W = args.steps, max(args.warmup, 3)
     p, phi, u, name = workload(args.config)
@@ -219,11 +216,8 @@ def run_acm(args, rank, local_rank, world):
     sim.profile(False)
     launches = sim.launch_count - launches0
     mass = sim.phi_mass()
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * N * K / (ms * 1e-3) / 1e6
+    ms = replicas.max_over_ranks(ms, dev)
+    value = replicas.aggregate_mlups(N, K, ms, world)
 
     # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region ----
     po, uo, pro = (torch.empty_like(phi_h).pin_memory(), torch.empty_like(u_h).pin_memory(),
@@ -237,11 +231,8 @@ def run_acm(args, rank, local_rank, world):
     t1.record()
     barrier()
     ms_e2e = t0.elapsed_time(t1)
-    if world > 1:
-        t = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
-    e2e = world * N * Ke / (ms_e2e * 1e-3) / 1e6
+    ms_e2e = replicas.max_over_ranks(ms_e2e, dev)
+    e2e = replicas.aggregate_mlups(N, Ke, ms_e2e, world)
     finite = bool(torch.isfinite(po).all() and torch.isfinite(uo).all())
 
     if rank == 0:
@@ -284,8 +275,7 @@ def run_acm(args, rank, local_rank, world):
             v, cores, sample, _, _ = oracle_sample(args.config, budget_s=15.0)
             out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
         print(json.dumps(out), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    replicas.shutdown()
 
 
 def main():

@@ -222,8 +222,20 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const P
     const T bz = p3 * uz + T(0.5) * tnz + k * dzm;
     const T p45 = T(4.5) * phi;
     T* dst = a.Hdst + idx;
-    emit_populations<Q, T>(A, bx, by, bz, p45 * ux * ux, p45 * uy * uy, p45 * uz * uz, p45 * ux * uy, p45 * ux * uz,
-                           p45 * uy * uz, [&](auto ic, T v) { st_stream(dst + (size_t) decltype(ic)::value * N, v); });
+    if constexpr (sizeof(T) == 8) {
+        emit_populations<Q, T>(A, bx, by, bz, p45 * ux * ux, p45 * uy * uy, p45 * uz * uz, p45 * ux * uy, p45 * ux * uz,
+                               p45 * uy * uz, [&](auto ic, T v) { st_stream(dst + (size_t) decltype(ic)::value * N, v); });
+    } else {
+        // fp32 instance (reading A22): the rest population is set by subtraction,
+        // h*_0 = phi_new - sum_{i>=1} h*_i, so that the collision conserves phi exactly in fp32.
+        T rest = phi;
+        emit_populations<Q, T>(A, bx, by, bz, p45 * ux * ux, p45 * uy * uy, p45 * uz * uz, p45 * ux * uy, p45 * ux * uz,
+                               p45 * uy * uz, [&](auto ic, T v) {
+                                   constexpr int i = decltype(ic)::value;
+                                   if constexpr (i > 0) { rest -= v; st_stream(dst + (size_t)i * N, v); }
+                               });
+        st_stream(dst, rest);
+    }
     a.Cdst[idx] = phi;
 }
 
