@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- MLUPS of the coupled fp64 ACM LB step (BASELINE.json metric) on B200.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl acm|reference] [--config 3]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl acm|reference] [--config 3] [--inplace]
 
 A "step" is one pass of the whole hot path (phase-field kernel + hydrodynamic kernel) over the
 whole grid of the workload.  The path does not shard (north_star: one GPU, no collectives):
@@ -193,7 +193,7 @@ def run_acm(args, rank, local_rank, world):
     np_dtype = "float64" if precision == "f64" else "float32"
     phi_h = torch.from_numpy(phi.astype(np_dtype)).pin_memory()
     u_h = torch.from_numpy(u.astype(np_dtype)).pin_memory()
-    sim = ACM.from_params(p, precision=precision, device=dev)
+    sim = ACM.from_params(p, precision=precision, device=dev, inplace=args.inplace)
     if args.block:
         sim.set_block(*args.block)
     sim.init(phi_h.to(dev), u_h.to(dev))
@@ -254,7 +254,7 @@ def run_acm(args, rank, local_rank, world):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": precision, "data": "synthetic",
-            "config": {"workload": name, "grid": [p.nx, p.ny, p.nz], "stencils": [p.stencil_phase, p.stencil_hydro],
+            "config": {"workload": name, "grid": [p.nx, p.ny, p.nz], "stencils": [p.stencil_phase, p.stencil_hydro], "streaming": "in-place AA" if args.inplace else "two-grid pull",
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": f"inputs larger than L2: {(2 * (p.stencil_phase + p.stencil_hydro) + 5) * N * esz / 1e9:.1f} GB "
                              "of state streamed every step vs 126 MB L2",
@@ -288,6 +288,7 @@ def main():
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--block", type=int, nargs=3, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--inplace", action="store_true", help="in-place AA streaming (one grid per population set)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

@@ -81,6 +81,21 @@ int acm_create(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int ste
                const double gravity[3], unsigned wall_flags, int precision,
                void* workspace, void* cuda_stream);
 
+/* Options of acm_create_opt / acm_workspace_bytes_opt (OR of):
+ *   ACM_OPT_INPLACE   one grid per population set instead of two (P:258 uses two): the streaming
+ *                     of h and g follows the in-place AA pattern the paper names as the open
+ *                     alternative; phi stays double-buffered because its finite-difference
+ *                     stencil is non-local.  Same results, same bytes moved per step, half the
+ *                     population memory. */
+enum { ACM_OPT_INPLACE = 1, ACM_OPT_ALL = 1 };
+size_t acm_workspace_bytes_opt(int nx, int ny, int nz, int stencil_phase, int stencil_hydro, int precision,
+                               unsigned options);
+/* acm_create with options; acm_create(...) == acm_create_opt(..., options = 0, ...). */
+int acm_create_opt(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int stencil_hydro,
+                   double rho_H, double rho_L, double sigma, double xi, double M, double nu_H, double nu_L,
+                   const double gravity[3], unsigned wall_flags, int precision, unsigned options,
+                   void* workspace, void* cuda_stream);
+
 /* Equilibrium initialiser ("Initialisation of all fields", Alg. 2 line 1):
  * phi-field <- phi, u-field <- u, h_i <- phi Gamma_i(u) (eq. 6), g_i <- Gamma_i(u) - w_i
  * (eq. 12 with p* = 0).  phi: [device] N values; u: [device] 3N values, component-major. */

@@ -15,8 +15,9 @@ from . import build as _build
 ACM_OK, ACM_EINVAL, ACM_ESTATE, ACM_ECUDA, ACM_EUNSTABLE = 0, 1, 2, 3, 4
 ACM_F64, ACM_F32 = 0, 1
 ACM_WALL_X, ACM_WALL_Y, ACM_WALL_Z = 1, 2, 4
+ACM_OPT_INPLACE = 1
 
-EXPORTS = ["acm_workspace_bytes", "acm_create", "acm_init", "acm_step", "acm_fields", "acm_phi_mass", "acm_get_pdfs",
+EXPORTS = ["acm_workspace_bytes", "acm_workspace_bytes_opt", "acm_create", "acm_create_opt", "acm_init", "acm_step", "acm_fields", "acm_phi_mass", "acm_get_pdfs",
            "acm_set_pdfs", "acm_run_host", "acm_set_block", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
 
 _lib = None
@@ -48,6 +49,9 @@ def load(build_if_missing: bool = True):
     lib.acm_workspace_bytes.restype = C.c_size_t
     lib.acm_workspace_bytes.argtypes = [i32] * 6
     lib.acm_create.argtypes = [C.POINTER(vp)] + [i32] * 5 + [dbl] * 7 + [C.POINTER(dbl), C.c_uint, i32, vp, vp]
+    lib.acm_workspace_bytes_opt.restype = C.c_size_t
+    lib.acm_workspace_bytes_opt.argtypes = [i32] * 6 + [C.c_uint]
+    lib.acm_create_opt.argtypes = [C.POINTER(vp)] + [i32] * 5 + [dbl] * 7 + [C.POINTER(dbl), C.c_uint, i32, C.c_uint, vp, vp]
     lib.acm_init.argtypes = [vp, vp, vp]
     lib.acm_step.argtypes = [vp, i32]
     lib.acm_fields.argtypes = [vp, vp, vp, vp]
@@ -81,7 +85,7 @@ class ACM:
 
     def __init__(self, nx, ny, nz, stencil_phase=15, stencil_hydro=19, rho_H=1.0, rho_L=1e-3, sigma=1e-4, xi=5.0,
                  M=0.02, nu_H=1 / 60, nu_L=1 / 60, gravity=(0.0, 0.0, 0.0), wall_flags=0, precision="f64",
-                 device="cuda:0", stream=None):
+                 device="cuda:0", stream=None, inplace=False):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2012_06144_b200 needs a CUDA device (no CPU fallback)")
         self._lib = load()
@@ -93,7 +97,9 @@ class ACM:
         self.precision = {"f64": ACM_F64, "f32": ACM_F32}[precision]
         self.dtype = torch.float64 if precision == "f64" else torch.float32
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-        nbytes = self._lib.acm_workspace_bytes(self.nx, self.ny, self.nz, self.Qh, self.Qg, self.precision)
+        self.options = ACM_OPT_INPLACE if inplace else 0
+        nbytes = self._lib.acm_workspace_bytes_opt(self.nx, self.ny, self.nz, self.Qh, self.Qg, self.precision,
+                                                   self.options)
         if nbytes == 0:
             raise AcmError(ACM_EINVAL, "invalid grid size / stencil / precision")
         with torch.cuda.device(self.device):
@@ -102,9 +108,9 @@ class ACM:
         g = (C.c_double * 3)(*[float(v) for v in gravity])
         h = C.c_void_p()
         with torch.cuda.device(self.device):
-            rc = self._lib.acm_create(C.byref(h), self.nx, self.ny, self.nz, self.Qh, self.Qg, rho_H, rho_L, sigma, xi,
-                                      M, nu_H, nu_L, g, int(wall_flags), self.precision, C.c_void_p(base),
-                                      C.c_void_p(self.stream.cuda_stream))
+            rc = self._lib.acm_create_opt(C.byref(h), self.nx, self.ny, self.nz, self.Qh, self.Qg, rho_H, rho_L, sigma,
+                                          xi, M, nu_H, nu_L, g, int(wall_flags), self.precision, self.options,
+                                          C.c_void_p(base), C.c_void_p(self.stream.cuda_stream))
         _check(self._lib, rc)
         self._h = h
 

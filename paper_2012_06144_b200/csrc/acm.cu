@@ -116,21 +116,74 @@ template <typename T> __device__ __forceinline__ void st_stream(T* p, T v)
 #endif
 }
 
-// Pull the Q populations arriving at this cell: f_i(x) <- F_i(x - e_i), or F_ibar(x) if x - e_i
-// lies beyond a wall (half-way bounce-back inside the streaming step).
-template <int Q, typename T, bool WALLS>
-__device__ __forceinline__ void pull(const T* __restrict__ F, size_t N, const Nbr& nb, T (&f)[Q])
+// ------------------------------------------------------------------------------------------
+// Storage states of a population array and the streaming they imply.
+//   ST_POST  (two-grid): slot i at x holds the post-collision f*_i(x); the next step pulls.
+//   ST_IN    (in place): slot i at x holds the incoming (streamed, pre-collision) f_i(x).
+//   ST_SWAP  (in place): slot ibar at x holds the post-collision f*_i(x) (directions swapped).
+// Two-grid update: ST_POST(src) -> ST_POST(dst).  In-place AA pattern (Bailey et al. 2009; the paper
+// names it P:52): even step ST_IN -> ST_SWAP touches only the own cell, odd step ST_SWAP -> ST_IN
+// reads slot ibar at x-e_i and writes slot i at x+e_i -- exactly the locations it read, so one array
+// suffices.  Half-way bounce-back: a population that would come from / go to a cell beyond a wall is
+// taken from / put into the opposite slot of the own cell.
+// ------------------------------------------------------------------------------------------
+enum { ST_POST = 0, ST_IN = 1, ST_SWAP = 2 };
+
+// incoming populations f_i(x) from an array in state STATE
+template <int Q, typename T, bool WALLS, int STATE>
+__device__ __forceinline__ void load_incoming(const T* F, size_t N, const Nbr& nb, T (&f)[Q])
 {
     using L = Lat<Q>;
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        constexpr int ex = L::ex(i), ey = L::ey(i), ez = L::ez(i);
-        const T* src = F + (size_t)i * N + nb.template at<-ex, -ey, -ez>();
-        if constexpr (WALLS && i > 0) {
-            if (nb.template beyond<-ex, -ey, -ez, WALLS>()) src = F + (size_t)L::opp(i) * N + nb.template at<0, 0, 0>();
+        constexpr int ex = L::ex(i), ey = L::ey(i), ez = L::ez(i), o = L::opp(i);
+        const T* src;
+        if constexpr (STATE == ST_IN) {
+            src = F + (size_t)i * N + nb.template at<0, 0, 0>();
+        } else {
+            constexpr int far = (STATE == ST_POST) ? i : o;      // slot at x - e_i
+            constexpr int own = (STATE == ST_POST) ? o : i;      // slot at x when x - e_i is beyond a wall
+            src = F + (size_t)far * N + nb.template at<-ex, -ey, -ez>();
+            if constexpr (WALLS && i > 0) {
+                if (nb.template beyond<-ex, -ey, -ez, WALLS>()) src = F + (size_t)own * N + nb.template at<0, 0, 0>();
+            }
         }
         f[i] = ld_stream(src);
     });
+}
+
+// address of the post-collision population f*_i(x) in the array the step writes.
+// FROM is the state the step read: ST_POST -> two-grid dst (ST_POST), ST_IN -> ST_SWAP, ST_SWAP -> ST_IN.
+template <int Q, int I, typename T, bool WALLS, int FROM>
+__device__ __forceinline__ T* outgoing_ptr(T* F, size_t N, const Nbr& nb)
+{
+    using L = Lat<Q>;
+    constexpr int ex = L::ex(I), ey = L::ey(I), ez = L::ez(I), o = L::opp(I);
+    if constexpr (FROM == ST_POST) {
+        return F + (size_t)I * N + nb.template at<0, 0, 0>();
+    } else if constexpr (FROM == ST_IN) {
+        return F + (size_t)o * N + nb.template at<0, 0, 0>();
+    } else {
+        T* dst = F + (size_t)I * N + nb.template at<ex, ey, ez>();
+        if constexpr (WALLS && I > 0) {
+            if (nb.template beyond<ex, ey, ez, WALLS>()) dst = F + (size_t)o * N + nb.template at<0, 0, 0>();
+        }
+        return dst;
+    }
+}
+
+// post-collision population f*_i(x) read back from an array in state STATE (export only)
+template <int Q, int I, typename T, int STATE>
+__device__ __forceinline__ T load_post(const T* F, size_t N, const Nbr& nb)
+{
+    using L = Lat<Q>;
+    constexpr int ex = L::ex(I), ey = L::ey(I), ez = L::ez(I), o = L::opp(I);
+    if constexpr (STATE == ST_POST) return F[(size_t)I * N + nb.template at<0, 0, 0>()];
+    else if constexpr (STATE == ST_SWAP) return F[(size_t)o * N + nb.template at<0, 0, 0>()];
+    else {
+        if (nb.template beyond<ex, ey, ez, true>()) return F[(size_t)o * N + nb.template at<0, 0, 0>()];
+        return F[(size_t)I * N + nb.template at<ex, ey, ez>()];
+    }
 }
 
 // Isotropic finite differences of phi on lattice Q (eqs. 23, 24 with c = dx = 1, c_s^2 = 1/3):
@@ -180,7 +233,7 @@ struct PhaseArgs {
     T one_minus_omega, inv_xi;
 };
 
-template <typename T, int Q, bool WALLS>
+template <typename T, int Q, bool WALLS, int STATE>
 __global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const PhaseArgs<T> a)
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
@@ -193,7 +246,7 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const P
     const size_t N = a.N;
 
     T h[Q];
-    pull<Q, T, WALLS>(a.Hsrc, N, nb, h);
+    load_incoming<Q, T, WALLS, STATE>(a.Hsrc, N, nb, h);
     const T ux = __ldg(a.U + idx), uy = __ldg(a.U + N + idx), uz = __ldg(a.U + 2 * N + idx);
     const T c0 = __ldg(a.Csrc + idx);
     T gx, gy, gz, lap_unused;
@@ -221,10 +274,11 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const P
     const T by = p3 * uy + T(0.5) * tny + k * dym;
     const T bz = p3 * uz + T(0.5) * tnz + k * dzm;
     const T p45 = T(4.5) * phi;
-    T* dst = a.Hdst + idx;
     if constexpr (sizeof(T) == 8) {
         emit_populations<Q, T>(A, bx, by, bz, p45 * ux * ux, p45 * uy * uy, p45 * uz * uz, p45 * ux * uy, p45 * ux * uz,
-                               p45 * uy * uz, [&](auto ic, T v) { st_stream(dst + (size_t) decltype(ic)::value * N, v); });
+                               p45 * uy * uz, [&](auto ic, T v) {
+                                   st_stream(outgoing_ptr<Q, decltype(ic)::value, T, WALLS, STATE>(a.Hdst, N, nb), v);
+                               });
     } else {
         // fp32 instance (reading A22): the rest population is set by subtraction,
         // h*_0 = phi_new - sum_{i>=1} h*_i, so that the collision conserves phi exactly in fp32.
@@ -232,9 +286,9 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const P
         emit_populations<Q, T>(A, bx, by, bz, p45 * ux * ux, p45 * uy * uy, p45 * uz * uz, p45 * ux * uy, p45 * ux * uz,
                                p45 * uy * uz, [&](auto ic, T v) {
                                    constexpr int i = decltype(ic)::value;
-                                   if constexpr (i > 0) { rest -= v; st_stream(dst + (size_t)i * N, v); }
+                                   if constexpr (i > 0) { rest -= v; st_stream(outgoing_ptr<Q, i, T, WALLS, STATE>(a.Hdst, N, nb), v); }
                                });
-        st_stream(dst, rest);
+        st_stream(outgoing_ptr<Q, 0, T, WALLS, STATE>(a.Hdst, N, nb), rest);
     }
     a.Cdst[idx] = phi;
 }
@@ -257,7 +311,7 @@ struct HydroArgs {
     T rho_L, drho, tau_L, dtau, beta4, kappa, gx, gy, gz;
 };
 
-template <typename T, int Q, bool WALLS>
+template <typename T, int Q, bool WALLS, int STATE>
 __global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const HydroArgs<T> a)
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
@@ -270,7 +324,7 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const H
     const size_t N = a.N;
 
     T g[Q];
-    pull<Q, T, WALLS>(a.Gsrc, N, nb, g);
+    load_incoming<Q, T, WALLS, STATE>(a.Gsrc, N, nb, g);
     const T uox = a.U[idx], uoy = a.U[N + idx], uoz = a.U[2 * N + idx];
     const T c0 = __ldg(a.C + idx);
     T gpx, gpy, gpz, lap;
@@ -312,15 +366,17 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const H
     const T Tyz = s45 * uy * uz + k45 * (m.Pyz - uy * uz);
     const T A = pstar - T(1.5) * (ux * ux + uy * uy + uz * uz) - T(1.5) * om * (nxx + nyy + nzz);
     const T bx = T(3) * (ux + hx), by = T(3) * (uy + hy), bz = T(3) * (uz + hz);
-    T* dst = a.Gdst + idx;
-    emit_populations<Q, T>(A, bx, by, bz, Txx, Tyy, Tzz, Txy, Txz, Tyz,
-                           [&](auto ic, T v) { st_stream(dst + (size_t) decltype(ic)::value * N, v); });
+    emit_populations<Q, T>(A, bx, by, bz, Txx, Tyy, Tzz, Txy, Txz, Tyz, [&](auto ic, T v) {
+        st_stream(outgoing_ptr<Q, decltype(ic)::value, T, WALLS, STATE>(a.Gdst, N, nb), v);
+    });
 }
 
 // ------------------------------------------------------------------------------------------
-// Equilibrium initialiser (Alg. 2 line 1): C <- phi, U <- u, h_i <- phi Gamma_i(u),
-// g_i <- Gamma_i(u) - w_i, the latter written in the "lazy pull" storage:
-//   Gs_i(y) = g_i(y + e_i), or g_ibar(y) if y + e_i lies beyond a wall.
+// Equilibrium initialiser (Alg. 2 line 1): C <- phi, U <- u, h*_i <- phi Gamma_i(u) (post-collision
+// convention: the first phase step streams it), g_i <- Gamma_i(u) - w_i (incoming convention: the
+// first hydrodynamic step collides it).  Storage: two-grid keeps both sets in ST_POST, so g is
+// pre-shifted (Gs_i(y) = g_i(y+e_i), or g_ibar(y) if y+e_i lies beyond a wall); in place h starts
+// in ST_SWAP and g in ST_IN.
 // ------------------------------------------------------------------------------------------
 template <int Q, typename T>
 __device__ __forceinline__ T gamma_i(int ex, int ey, int ez, T w, T ux, T uy, T uz)
@@ -329,7 +385,7 @@ __device__ __forceinline__ T gamma_i(int ex, int ey, int ez, T w, T ux, T uy, T 
     return w * (T(1) + T(3) * eu + T(4.5) * eu * eu - T(1.5) * (ux * ux + uy * uy + uz * uz));
 }
 
-template <typename T, int QH, int QG>
+template <typename T, int QH, int QG, bool INPLACE>
 __global__ void init_kernel(const T* __restrict__ phi, const T* __restrict__ u, T* H, T* G, T* C, T* U, Geom g, size_t N)
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
@@ -346,14 +402,17 @@ __global__ void init_kernel(const T* __restrict__ phi, const T* __restrict__ u, 
     static_for<0, QH>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
         using L = Lat<QH>;
-        H[(size_t)i * N + idx] = ph * gamma_i<QH, T>(L::ex(i), L::ey(i), L::ez(i), T(L::w(i)), ux, uy, uz);
+        constexpr int slot = INPLACE ? L::opp(i) : i;
+        H[(size_t)slot * N + idx] = ph * gamma_i<QH, T>(L::ex(i), L::ey(i), L::ez(i), T(L::w(i)), ux, uy, uz);
     });
     static_for<0, QG>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
         using L = Lat<QG>;
         constexpr int ex = L::ex(i), ey = L::ey(i), ez = L::ez(i);
         T v;
-        if (nb.template beyond<ex, ey, ez, true>()) {
+        if constexpr (INPLACE) {
+            v = gamma_i<QG, T>(ex, ey, ez, T(L::w(i)), ux, uy, uz) - T(L::w(i));
+        } else if (nb.template beyond<ex, ey, ez, true>()) {
             constexpr int o = L::opp(i);
             v = gamma_i<QG, T>(L::ex(o), L::ey(o), L::ez(o), T(L::w(o)), ux, uy, uz) - T(L::w(o));
         } else {
@@ -365,11 +424,12 @@ __global__ void init_kernel(const T* __restrict__ phi, const T* __restrict__ u, 
 }
 
 // ------------------------------------------------------------------------------------------
-// Diagnostics and debug export
+// Diagnostics and debug export / import
 // ------------------------------------------------------------------------------------------
-// out_i(x) = pulled G (applies the pending streaming); also p = c_s^2 rho(phi) sum_i g_i
-template <typename T, int Q>
-__global__ void gather_g_kernel(const T* __restrict__ Gs, const T* __restrict__ C, T* out, T* p, Geom g, size_t N, T rho_L, T drho)
+// Export of a population array stored in state STATE, in the convention POST (post-collision value at
+// its own cell) or incoming (streamed value); optionally p = c_s^2 rho(phi) sum_i f_i.
+template <typename T, int Q, int STATE, bool POST>
+__global__ void export_kernel(const T* F, const T* __restrict__ C, T* out, T* p, Geom g, size_t N, T rho_L, T drho)
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -379,7 +439,8 @@ __global__ void gather_g_kernel(const T* __restrict__ Gs, const T* __restrict__ 
     nb.setup<true>(g, x, y, z);
     const int idx = nb.at<0, 0, 0>();
     T f[Q];
-    pull<Q, T, true>(Gs, N, nb, f);
+    if constexpr (POST) static_for<0, Q>([&](auto ic) { constexpr int i = decltype(ic)::value; f[i] = load_post<Q, i, T, STATE>(F, N, nb); });
+    else load_incoming<Q, T, true, STATE>(F, N, nb, f);
     if (out) static_for<0, Q>([&](auto ic) { constexpr int i = decltype(ic)::value; out[(size_t)i * N + idx] = f[i]; });
     if (p) {
         Moments<Q, T, false> m;
@@ -388,9 +449,11 @@ __global__ void gather_g_kernel(const T* __restrict__ Gs, const T* __restrict__ 
     }
 }
 
-// inverse of gather_g_kernel: Gs_i(y) = g_i(y+e_i) or g_ibar(y) behind a wall
-template <typename T, int Q>
-__global__ void scatter_g_kernel(const T* __restrict__ gin, T* Gs, Geom g, size_t N)
+// Import: POST convention -> ST_SWAP storage (local permutation), or incoming convention -> ST_POST
+// storage (Fs_i(y) = f_i(y+e_i), or f_ibar(y) if y+e_i lies beyond a wall).  The other two cases
+// (POST -> ST_POST, incoming -> ST_IN) are plain copies.
+template <typename T, int Q, bool POST>
+__global__ void import_kernel(const T* __restrict__ in, T* F, Geom g, size_t N)
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -403,9 +466,13 @@ __global__ void scatter_g_kernel(const T* __restrict__ gin, T* Gs, Geom g, size_
         constexpr int i = decltype(ic)::value;
         using L = Lat<Q>;
         constexpr int ex = L::ex(i), ey = L::ey(i), ez = L::ez(i);
-        const T v = nb.template beyond<ex, ey, ez, true>() ? gin[(size_t)L::opp(i) * N + idx]
-                                                           : gin[(size_t)i * N + nb.template at<ex, ey, ez>()];
-        Gs[(size_t)i * N + idx] = v;
+        if constexpr (POST) {
+            F[(size_t)L::opp(i) * N + idx] = in[(size_t)i * N + idx];
+        } else {
+            const T v = nb.template beyond<ex, ey, ez, true>() ? in[(size_t)L::opp(i) * N + idx]
+                                                               : in[(size_t)i * N + nb.template at<ex, ey, ez>()];
+            F[(size_t)i * N + idx] = v;
+        }
     });
 }
 
@@ -473,6 +540,8 @@ struct acm_ctx {
     // carved workspace (byte offsets)
     size_t offH[2], offG[2], offC[2], offU, offStage, offRed;
     int curH, curG, curC;       // which buffer holds the current state
+    unsigned options;           // ACM_OPT_*
+    int stH, stG;               // storage state of the current H / G buffer (ST_POST | ST_IN | ST_SWAP)
     bool initialised;
     int sticky;                 // ACM_OK or ACM_ECUDA
     dim3 block;
@@ -491,16 +560,19 @@ struct Layout {
     size_t offH[2], offG[2], offC[2], offU, offStage, offRed, total;
 };
 
-static bool make_layout(int nx, int ny, int nz, int Qh, int Qg, int precision, Layout* L)
+static bool make_layout(int nx, int ny, int nz, int Qh, int Qg, int precision, unsigned options, Layout* L)
 {
+    if (options & ~(unsigned)ACM_OPT_ALL) return false;
+    const int grids = (options & ACM_OPT_INPLACE) ? 1 : 2;
     if (nx <= 0 || ny <= 0 || nz <= 0 || !valid_stencil(Qh) || !valid_stencil(Qg)) return false;
     if (precision != ACM_F64 && precision != ACM_F32) return false;
     const double cells = (double)nx * ny * nz;
     if (cells >= 2147483648.0) return false;
     const size_t N = (size_t)nx * ny * nz, e = precision == ACM_F64 ? 8 : 4;
     size_t o = 0;
-    for (int b = 0; b < 2; ++b) { L->offH[b] = o; o = align256(o + (size_t)Qh * N * e); }
-    for (int b = 0; b < 2; ++b) { L->offG[b] = o; o = align256(o + (size_t)Qg * N * e); }
+    for (int b = 0; b < grids; ++b) { L->offH[b] = o; o = align256(o + (size_t)Qh * N * e); }
+    for (int b = 0; b < grids; ++b) { L->offG[b] = o; o = align256(o + (size_t)Qg * N * e); }
+    if (grids == 1) { L->offH[1] = L->offH[0]; L->offG[1] = L->offG[0]; }
     for (int b = 0; b < 2; ++b) { L->offC[b] = o; o = align256(o + N * e); }
     L->offU = o; o = align256(o + 3 * N * e);
     L->offStage = o; o = align256(o + 5 * N * e);
@@ -532,12 +604,35 @@ template <typename T, int QH, int QG>
 static int do_init(acm_ctx* c, const T* phi, const T* u)
 {
     Geom g{c->nx, c->ny, c->nz, c->walls};
-    dim3 b(128, 1, 1);
-    init_kernel<T, QH, QG><<<grid_for(c, b), b, 0, c->stream>>>(phi, u, wsp<T>(c, c->offH[0]), wsp<T>(c, c->offG[0]),
-                                                                 wsp<T>(c, c->offC[0]), wsp<T>(c, c->offU), g, c->N);
+    dim3 b(128, 1, 1), gr = grid_for(c, b);
+    T *H = wsp<T>(c, c->offH[0]), *G = wsp<T>(c, c->offG[0]), *C = wsp<T>(c, c->offC[0]), *U = wsp<T>(c, c->offU);
+    if (c->options & ACM_OPT_INPLACE) {
+        init_kernel<T, QH, QG, true><<<gr, b, 0, c->stream>>>(phi, u, H, G, C, U, g, c->N);
+        c->stH = ST_SWAP; c->stG = ST_IN;
+    } else {
+        init_kernel<T, QH, QG, false><<<gr, b, 0, c->stream>>>(phi, u, H, G, C, U, g, c->N);
+        c->stH = c->stG = ST_POST;
+    }
     c->curH = c->curG = c->curC = 0;
     return check_launch(c, "init_kernel");
 }
+
+// launches K<T, Q, WALLS, STATE> for the runtime (walls, state) pair
+#define ACM_LAUNCH_STATE(KERNEL, TT, QQ, walls, state, gr, b, stream, args)                          \
+    do {                                                                                              \
+        if (walls) {                                                                                  \
+            if (state == ST_POST) KERNEL<TT, QQ, true, ST_POST><<<gr, b, 0, stream>>>(args);          \
+            else if (state == ST_IN) KERNEL<TT, QQ, true, ST_IN><<<gr, b, 0, stream>>>(args);         \
+            else KERNEL<TT, QQ, true, ST_SWAP><<<gr, b, 0, stream>>>(args);                           \
+        } else {                                                                                      \
+            if (state == ST_POST) KERNEL<TT, QQ, false, ST_POST><<<gr, b, 0, stream>>>(args);         \
+            else if (state == ST_IN) KERNEL<TT, QQ, false, ST_IN><<<gr, b, 0, stream>>>(args);        \
+            else KERNEL<TT, QQ, false, ST_SWAP><<<gr, b, 0, stream>>>(args);                          \
+        }                                                                                             \
+    } while (0)
+
+// state of the array after a step that read it in state s
+static int next_state(int s) { return s == ST_POST ? ST_POST : (s == ST_IN ? ST_SWAP : ST_IN); }
 
 template <typename T, int QH>
 static int launch_phase(acm_ctx* c)
@@ -552,9 +647,9 @@ static int launch_phase(acm_ctx* c)
     a.one_minus_omega = (T)(1.0 - omega);
     a.inv_xi = (T)(1.0 / c->xi);
     dim3 b = c->block, gr = grid_for(c, b);
-    if (c->walls) phase_kernel<T, QH, true><<<gr, b, 0, c->stream>>>(a);
-    else phase_kernel<T, QH, false><<<gr, b, 0, c->stream>>>(a);
+    ACM_LAUNCH_STATE(phase_kernel, T, QH, c->walls, c->stH, gr, b, c->stream, a);
     c->curH ^= 1; c->curC ^= 1;
+    c->stH = next_state(c->stH);
     return check_launch(c, "phase_kernel");
 }
 
@@ -572,29 +667,33 @@ static int launch_hydro(acm_ctx* c)
     a.beta4 = (T)(4.0 * 12.0 * c->sigma / c->xi); a.kappa = (T)(1.5 * c->sigma * c->xi);
     a.gx = (T)c->grav[0]; a.gy = (T)c->grav[1]; a.gz = (T)c->grav[2];
     dim3 b = c->block, gr = grid_for(c, b);
-    if (c->walls) hydro_kernel<T, QG, true><<<gr, b, 0, c->stream>>>(a);
-    else hydro_kernel<T, QG, false><<<gr, b, 0, c->stream>>>(a);
+    ACM_LAUNCH_STATE(hydro_kernel, T, QG, c->walls, c->stG, gr, b, c->stream, a);
     c->curG ^= 1;
+    c->stG = next_state(c->stG);
     return check_launch(c, "hydro_kernel");
 }
 
-template <typename T, int QG>
-static int do_gather(acm_ctx* c, T* gout, T* p)
+// export of H (post-collision convention) or G (incoming convention, optionally p) from the current state
+template <typename T, int Q, bool POST>
+static int do_export(acm_ctx* c, const T* F, int state, T* out, T* p)
 {
     Geom g{c->nx, c->ny, c->nz, c->walls};
-    dim3 b(128, 1, 1);
-    gather_g_kernel<T, QG><<<grid_for(c, b), b, 0, c->stream>>>(wsp<T>(c, c->offG[c->curG]), wsp<T>(c, c->offC[c->curC]), gout, p,
-                                                               g, c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L));
-    return check_launch(c, "gather_g_kernel");
+    dim3 b(128, 1, 1), gr = grid_for(c, b);
+    const T* C = wsp<T>(c, c->offC[c->curC]);
+    const T rl = (T)c->rho_L, dr = (T)(c->rho_H - c->rho_L);
+    if (state == ST_POST) export_kernel<T, Q, ST_POST, POST><<<gr, b, 0, c->stream>>>(F, C, out, p, g, c->N, rl, dr);
+    else if (state == ST_IN) export_kernel<T, Q, ST_IN, POST><<<gr, b, 0, c->stream>>>(F, C, out, p, g, c->N, rl, dr);
+    else export_kernel<T, Q, ST_SWAP, POST><<<gr, b, 0, c->stream>>>(F, C, out, p, g, c->N, rl, dr);
+    return check_launch(c, "export_kernel");
 }
 
-template <typename T, int QG>
-static int do_scatter(acm_ctx* c, const T* gin)
+template <typename T, int Q, bool POST>
+static int do_import(acm_ctx* c, const T* in, T* F)
 {
     Geom g{c->nx, c->ny, c->nz, c->walls};
     dim3 b(128, 1, 1);
-    scatter_g_kernel<T, QG><<<grid_for(c, b), b, 0, c->stream>>>(gin, wsp<T>(c, c->offG[c->curG]), g, c->N);
-    return check_launch(c, "scatter_g_kernel");
+    import_kernel<T, Q, POST><<<grid_for(c, b), b, 0, c->stream>>>(in, F, g, c->N);
+    return check_launch(c, "import_kernel");
 }
 
 // ---- dispatch over (precision, stencils) ---------------------------------------------------
@@ -639,18 +738,34 @@ static int step_t(acm_ctx* c, int n)
 }
 
 template <typename T>
-static int gather_t(acm_ctx* c, void* g, void* p)
+static int export_g_t(acm_ctx* c, void* g, void* p)
 {
     int rc = ACM_OK;
-    ACM_DISPATCH_Q(c->Qg, QG, rc = (do_gather<T, QG>(c, (T*)g, (T*)p)));
+    ACM_DISPATCH_Q(c->Qg, QG, rc = (do_export<T, QG, false>(c, wsp<T>(c, c->offG[c->curG]), c->stG, (T*)g, (T*)p)));
     return rc;
 }
 
 template <typename T>
-static int scatter_t(acm_ctx* c, const void* g)
+static int export_h_t(acm_ctx* c, void* h)
 {
     int rc = ACM_OK;
-    ACM_DISPATCH_Q(c->Qg, QG, rc = (do_scatter<T, QG>(c, (const T*)g)));
+    ACM_DISPATCH_Q(c->Qh, QH, rc = (do_export<T, QH, true>(c, wsp<T>(c, c->offH[c->curH]), c->stH, (T*)h, (T*)nullptr)));
+    return rc;
+}
+
+template <typename T>
+static int import_g_t(acm_ctx* c, const void* g)      // incoming convention -> ST_POST storage
+{
+    int rc = ACM_OK;
+    ACM_DISPATCH_Q(c->Qg, QG, rc = (do_import<T, QG, false>(c, (const T*)g, wsp<T>(c, c->offG[c->curG]))));
+    return rc;
+}
+
+template <typename T>
+static int import_h_t(acm_ctx* c, const void* h)      // post-collision convention -> ST_SWAP storage
+{
+    int rc = ACM_OK;
+    ACM_DISPATCH_Q(c->Qh, QH, rc = (do_import<T, QH, true>(c, (const T*)h, wsp<T>(c, c->offH[c->curH]))));
     return rc;
 }
 
@@ -675,20 +790,33 @@ const char* acm_last_error(void) { return g_err; }
 
 size_t acm_workspace_bytes(int nx, int ny, int nz, int stencil_phase, int stencil_hydro, int precision)
 {
+    return acm_workspace_bytes_opt(nx, ny, nz, stencil_phase, stencil_hydro, precision, 0u);
+}
+
+size_t acm_workspace_bytes_opt(int nx, int ny, int nz, int stencil_phase, int stencil_hydro, int precision, unsigned options)
+{
     Layout L;
-    return make_layout(nx, ny, nz, stencil_phase, stencil_hydro, precision, &L) ? L.total : 0;
+    return make_layout(nx, ny, nz, stencil_phase, stencil_hydro, precision, options, &L) ? L.total : 0;
 }
 
 int acm_create(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int stencil_hydro, double rho_H, double rho_L,
                double sigma, double xi, double M, double nu_H, double nu_L, const double gravity[3], unsigned wall_flags,
                int precision, void* workspace, void* cuda_stream)
 {
+    return acm_create_opt(out, nx, ny, nz, stencil_phase, stencil_hydro, rho_H, rho_L, sigma, xi, M, nu_H, nu_L, gravity,
+                          wall_flags, precision, 0u, workspace, cuda_stream);
+}
+
+int acm_create_opt(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int stencil_hydro, double rho_H, double rho_L,
+                   double sigma, double xi, double M, double nu_H, double nu_L, const double gravity[3], unsigned wall_flags,
+                   int precision, unsigned options, void* workspace, void* cuda_stream)
+{
     if (!out) return fail(ACM_EINVAL, "acm_create: out is NULL");
     *out = nullptr;
     Layout L;
-    if (!make_layout(nx, ny, nz, stencil_phase, stencil_hydro, precision, &L))
-        return fail(ACM_EINVAL, "acm_create: invalid size (%d,%d,%d), stencils (%d,%d) or precision %d", nx, ny, nz,
-                    stencil_phase, stencil_hydro, precision);
+    if (!make_layout(nx, ny, nz, stencil_phase, stencil_hydro, precision, options, &L))
+        return fail(ACM_EINVAL, "acm_create: invalid size (%d,%d,%d), stencils (%d,%d), precision %d or options %u", nx, ny, nz,
+                    stencil_phase, stencil_hydro, precision, options);
     if (!(rho_L > 0.0) || !(rho_H >= rho_L)) return fail(ACM_EINVAL, "acm_create: need rho_H >= rho_L > 0");
     if (!(xi > 0.0)) return fail(ACM_EINVAL, "acm_create: need xi > 0");
     if (!(sigma >= 0.0)) return fail(ACM_EINVAL, "acm_create: need sigma >= 0");
@@ -709,6 +837,8 @@ int acm_create(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int ste
     for (int b = 0; b < 2; ++b) { c->offH[b] = L.offH[b]; c->offG[b] = L.offG[b]; c->offC[b] = L.offC[b]; }
     c->offU = L.offU; c->offStage = L.offStage; c->offRed = L.offRed;
     c->curH = c->curG = c->curC = 0;
+    c->options = options;
+    c->stH = c->stG = ST_POST;
     c->initialised = false;
     c->sticky = ACM_OK;
     c->block = dim3(128, 1, 1);
@@ -801,7 +931,7 @@ int acm_fields(acm_ctx* c, void* phi, void* u, void* p)
     int rc = ACM_OK;
     if (phi) rc = copy_async(c, phi, c->ws + c->offC[c->curC], c->N * c->esz, cudaMemcpyDeviceToDevice, "acm_fields(phi)");
     if (!rc && u) rc = copy_async(c, u, c->ws + c->offU, 3 * c->N * c->esz, cudaMemcpyDeviceToDevice, "acm_fields(u)");
-    if (!rc && p) rc = c->precision == ACM_F64 ? gather_t<double>(c, nullptr, p) : gather_t<float>(c, nullptr, p);
+    if (!rc && p) rc = c->precision == ACM_F64 ? export_g_t<double>(c, nullptr, p) : export_g_t<float>(c, nullptr, p);
     return rc;
 }
 
@@ -833,8 +963,8 @@ int acm_get_pdfs(acm_ctx* c, void* h, void* g)
     ACM_CHECK_CTX(c);
     if (!c->initialised) return fail(ACM_ESTATE, "acm_get_pdfs: call acm_init first");
     int rc = ACM_OK;
-    if (h) rc = copy_async(c, h, c->ws + c->offH[c->curH], (size_t)c->Qh * c->N * c->esz, cudaMemcpyDeviceToDevice, "acm_get_pdfs(h)");
-    if (!rc && g) rc = c->precision == ACM_F64 ? gather_t<double>(c, g, nullptr) : gather_t<float>(c, g, nullptr);
+    if (h) rc = c->precision == ACM_F64 ? export_h_t<double>(c, h) : export_h_t<float>(c, h);
+    if (!rc && g) rc = c->precision == ACM_F64 ? export_g_t<double>(c, g, nullptr) : export_g_t<float>(c, g, nullptr);
     return rc;
 }
 
@@ -843,8 +973,17 @@ int acm_set_pdfs(acm_ctx* c, const void* h, const void* g)
     ACM_CHECK_CTX(c);
     if (!c->initialised) return fail(ACM_ESTATE, "acm_set_pdfs: call acm_init first");
     int rc = ACM_OK;
-    if (h) rc = copy_async(c, c->ws + c->offH[c->curH], h, (size_t)c->Qh * c->N * c->esz, cudaMemcpyDeviceToDevice, "acm_set_pdfs(h)");
-    if (!rc && g) rc = c->precision == ACM_F64 ? scatter_t<double>(c, g) : scatter_t<float>(c, g);
+    const bool inplace = (c->options & ACM_OPT_INPLACE) != 0;
+    if (h) {
+        // post-collision convention: two-grid stores it as is (ST_POST); in place as ST_SWAP
+        if (inplace) { rc = c->precision == ACM_F64 ? import_h_t<double>(c, h) : import_h_t<float>(c, h); c->stH = ST_SWAP; }
+        else rc = copy_async(c, c->ws + c->offH[c->curH], h, (size_t)c->Qh * c->N * c->esz, cudaMemcpyDeviceToDevice, "acm_set_pdfs(h)");
+    }
+    if (!rc && g) {
+        // incoming convention: in place stores it as is (ST_IN); two-grid pre-shifts it into ST_POST
+        if (inplace) { rc = copy_async(c, c->ws + c->offG[c->curG], g, (size_t)c->Qg * c->N * c->esz, cudaMemcpyDeviceToDevice, "acm_set_pdfs(g)"); c->stG = ST_IN; }
+        else rc = c->precision == ACM_F64 ? import_g_t<double>(c, g) : import_g_t<float>(c, g);
+    }
     return rc;
 }
 

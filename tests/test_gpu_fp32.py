@@ -98,7 +98,7 @@ def test_fp32_full_size_sampled_256():
         o.step(1)
         ho, go = o.get_pdfs()
         po, uo, _ = o.fields(False)
-        assert np.abs(h1[:, iz, iy, ix].cpu().numpy()[sl] - ho[sl]).max() < 2e-7
+        assert np.abs(h1[:, iz, iy, ix].cpu().numpy()[sl] - ho[sl]).max() < 1e-6      # rest population: 26 subtractions
         assert np.abs(g1[:, iz, iy, ix].cpu().numpy()[sl] - go[sl]).max() < 2e-7
         assert np.abs(c1[iz, iy, ix].cpu().numpy()[inner] - po[inner]).max() < 5e-7
         assert np.abs(u1[:, iz, iy, ix].cpu().numpy()[sl] - uo[sl]).max() < 2e-6

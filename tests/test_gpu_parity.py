@@ -62,29 +62,32 @@ ONE_STEP = [
 ]
 
 
+@pytest.mark.parametrize("inplace", [False, True])
 @pytest.mark.parametrize("nx,ny,nz,Qh,Qg,walls,grav,block", ONE_STEP)
-def test_one_step_pdf_parity(nx, ny, nz, Qh, Qg, walls, grav, block):
-    """One coupled step from a random non-equilibrium state: every population within 1e-13."""
+def test_one_step_pdf_parity(nx, ny, nz, Qh, Qg, walls, grav, block, inplace):
+    """One coupled step from a random non-equilibrium state: every population within 1e-13
+    (two-grid and in-place AA streaming; the second step covers the other AA kernel parity)."""
     p = Params(nx=nx, ny=ny, nz=nz, stencil_phase=Qh, stencil_hydro=Qg, wall_flags=walls, gravity=grav,
                rho_H=1.0, rho_L=1e-3, sigma=1e-4, nu_H=0.05, nu_L=1 / 60)
     phi, u, h, g = random_state(p, seed=11)
     o = Oracle.from_params(p)
     o.init(phi, u)
     o.set_pdfs(h, g)
-    a = _acm(p)
+    a = _acm(p, inplace=inplace)
     a.set_block(*block)
     a.init(_dev(phi), _dev(u))
     a.set_pdfs(_dev(h), _dev(g))
-    # set/get round trip is exact (g goes through the lazy-pull scatter/gather)
+    # set/get round trip is exact (the populations go through the storage-state import/export)
     h0, g0 = a.get_pdfs()
     assert (h0.cpu().numpy() == h).all() and (g0.cpu().numpy() == g).all()
-    o.step(1)
-    a.step(1)
-    ho, go = o.get_pdfs()
-    ha, ga = a.get_pdfs()
-    assert np.abs(ha.cpu().numpy() - ho).max() <= TOL_PDF_1STEP
-    assert np.abs(ga.cpu().numpy() - go).max() <= TOL_PDF_1STEP
-    _compare_fields(o, a, TOL_PDF_1STEP)
+    for k in (1, 2):
+        o.step(1)
+        a.step(1)
+        ho, go = o.get_pdfs()
+        ha, ga = a.get_pdfs()
+        assert np.abs(ha.cpu().numpy() - ho).max() <= k * TOL_PDF_1STEP
+        assert np.abs(ga.cpu().numpy() - go).max() <= k * TOL_PDF_1STEP
+        _compare_fields(o, a, k * TOL_PDF_1STEP)
 
 
 def test_init_parity():
@@ -167,8 +170,9 @@ def test_config5_scaled_q27_50_steps():
     _compare_fields(o, a, TOL_FIELD_100)
 
 
+@pytest.mark.parametrize("inplace", [False, True])
 @pytest.mark.parametrize("shape", [(1, 1, 1), (2, 1, 3), (1, 5, 1), (3, 2, 2)])
-def test_degenerate_grids(shape):
+def test_degenerate_grids(shape, inplace):
     """Tiny grids where a cell is its own periodic neighbour."""
     nx, ny, nz = shape
     p = Params(nx=nx, ny=ny, nz=nz, stencil_phase=27, stencil_hydro=27)
@@ -176,7 +180,7 @@ def test_degenerate_grids(shape):
     o = Oracle.from_params(p)
     o.init(phi, u)
     o.set_pdfs(h, g)
-    a = _acm(p)
+    a = _acm(p, inplace=inplace)
     a.init(_dev(phi), _dev(u))
     a.set_pdfs(_dev(h), _dev(g))
     o.step(3)
@@ -185,6 +189,41 @@ def test_degenerate_grids(shape):
     ha, ga = a.get_pdfs()
     assert np.abs(ha.cpu().numpy() - ho).max() <= 1e-12
     assert np.abs(ga.cpu().numpy() - go).max() <= 1e-12
+
+
+@pytest.mark.parametrize("case", ["config1", "walls", "config3"])
+def test_inplace_streaming_100_steps(case):
+    """in-place (AA-pattern) streaming of h and g, phi double-buffered.  Same
+    bar as the two-grid path: phi, u, p within 1e-10 of the oracle after 99 and 100 steps (odd and
+    even step counts end in different storage states), init parity, half the population memory."""
+    from paper_2012_06144_b200 import binding
+    if case == "config1":
+        p, phi, u = inputs.config1()
+    elif case == "walls":
+        p = Params(nx=24, ny=20, nz=28, gravity=(0.0, -1e-6, 0.0), wall_flags=inputs.WALL_X | inputs.WALL_Y | inputs.WALL_Z)
+        phi, u = inputs.sphere_phi(p, (12.0, 9.0, 14.0), 6.0, heavy_inside=True), inputs.zeros_u(p)
+    else:
+        p, phi, u = inputs.scaled_config3(40)
+    o = Oracle.from_params(p)
+    o.init(phi, u)
+    a = _acm(p, inplace=True)
+    a.init(_dev(phi), _dev(u))
+    ho, go = o.get_pdfs()
+    ha, ga = a.get_pdfs()
+    assert np.abs(ha.cpu().numpy() - ho).max() <= 1e-15 and np.abs(ga.cpu().numpy() - go).max() <= 1e-15
+    o.step(99)
+    a.step(99)
+    _compare_fields(o, a, TOL_FIELD_100)
+    o.step(1)
+    a.step(1)
+    _compare_fields(o, a, TOL_FIELD_100)
+    ho, go = o.get_pdfs()
+    ha, ga = a.get_pdfs()
+    assert np.abs(ha.cpu().numpy() - ho).max() <= TOL_FIELD_100 and np.abs(ga.cpu().numpy() - go).max() <= TOL_FIELD_100
+    lib = binding.load()
+    two = lib.acm_workspace_bytes_opt(p.nx, p.ny, p.nz, 15, 19, 0, 0)
+    one = lib.acm_workspace_bytes_opt(p.nx, p.ny, p.nz, 15, 19, 0, binding.ACM_OPT_INPLACE)
+    assert two - one >= (15 + 19) * p.ncells * 8
 
 
 def test_step_zero_and_state_errors():
