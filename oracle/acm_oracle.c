@@ -35,6 +35,8 @@
  *   A17 F_b = rho(phi) * gravity (no hydrostatic subtraction)
  *   A18 no clamp on phi or rho
  *   A19 p = p* rho c_s^2
+ *   A23 variant ORACLE_VAR_PHASE_SRT: Omega^h = omega_phi I
+ *   A24 bubble volume/centroid/velocity weighted with (1 - phi)
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): lattice identities, weighted
  * orthogonality of M, eq.25 forcing identity, brute-force 4^3 step against a
@@ -90,7 +92,13 @@ typedef struct oracle_ctx {
     double omega_phi, beta, kappa, tau_H, tau_L;
     double *H, *H2, *G, *G2, *C, *C2, *U, *U2, *tmp;
     int initialised;
+    unsigned variant;         /* ORACLE_VAR_* */
 } oracle_ctx;
+
+/* Variants of the operators the paper itself uses elsewhere:
+ *   ORACLE_VAR_PHASE_SRT  single-relaxation-time phase-field collision, Omega^h = omega_phi I
+ *                         ("a D3Q15 SRT LB scheme for the interface tracking"), reading A23 */
+enum { ORACLE_VAR_PHASE_SRT = 1 };
 
 /* ------------------------------------------------------------------------- */
 /* Lattices and moment matrices                                               */
@@ -328,9 +336,11 @@ static void phase_step(oracle_ctx *o)
                     heq[i] = phin[c] * Gamma(L, i, u);                           /* P:83 */
                     d[i] = heq[i] - ht[i * N + c] - 0.5 * F[i];
                 }
-                /* Omega d = M^-1 S M d ; S: first-order moments omega_phi, others 1 (A2, A3) */
+                /* Omega d = M^-1 S M d ; S: first-order moments omega_phi, others 1 (A2, A3);
+                 * SRT variant (P:285, A23): every moment relaxes with omega_phi */
+                const int srt = (o->variant & ORACLE_VAR_PHASE_SRT) != 0;
                 matvec(Q, L->M, d, m);
-                for (int k = 0; k < Q; ++k) m[k] *= (L->order[k] == 1) ? o->omega_phi : 1.0;
+                for (int k = 0; k < Q; ++k) m[k] *= (srt || L->order[k] == 1) ? o->omega_phi : 1.0;
                 matvec(Q, L->Minv, m, r);
                 for (int i = 0; i < Q; ++i) o->tmp[i * N + c] = r[i] + ht[i * N + c] + F[i];   /* eq. 4 */
             }
@@ -584,6 +594,70 @@ int oracle_fd(oracle_ctx *o, int use_hydro_stencil, const double *C, double *gra
                 if (lap) lap[c] = lap_phi(o, L, C, x, y, z);
             }
     return 0;
+}
+
+int oracle_set_variant(oracle_ctx *o, unsigned flags)
+{
+    if (!o || (flags & ~(unsigned)ORACLE_VAR_PHASE_SRT)) return 1;
+    o->variant = flags;
+    return 0;
+}
+
+/* Rising-bubble diagnostics (section 6.1).  The paper uses "the terminal velocity of the
+ * bubbles" u_t in eq. 34 without saying how it is measured; reading A24: the light
+ * phase is weighted with (phi_H - phi), i.e.
+ *   V = sum_x (1 - phi),  X_b = sum_x (1 - phi) x_c / V,  u_b = sum_x (1 - phi) u / V,
+ * x_c = cell centre (i + 1/2), plain coordinates (no periodic unwrapping).
+ * out = { V, X_b[3], u_b[3] }. */
+int oracle_bubble_diag(oracle_ctx *o, double out[7])
+{
+    if (!o || !out) return 1;
+    const size_t N = o->N;
+    double V = 0.0, X[3] = {0, 0, 0}, Ub[3] = {0, 0, 0};
+    for (int z = 0; z < o->nz; ++z)
+        for (int y = 0; y < o->ny; ++y)
+            for (int x = 0; x < o->nx; ++x) {
+                size_t c = cell(o, x, y, z);
+                double wgt = PHI_H - o->C[c];
+                V += wgt;
+                X[0] += wgt * (x + 0.5); X[1] += wgt * (y + 0.5); X[2] += wgt * (z + 0.5);
+                for (int a = 0; a < 3; ++a) Ub[a] += wgt * o->U[a * N + c];
+            }
+    out[0] = V;
+    for (int a = 0; a < 3; ++a) { out[1 + a] = X[a] / V; out[4 + a] = Ub[a] / V; }
+    return 0;
+}
+
+/* Dimensionless groups of section 6.1 solved for the lattice parameters:
+ *   t_ref = sqrt(D/g_y)                 (eq. 33)  =>  g_y   = D / t_ref^2
+ *   Eo    = g_y rho_H D^2 / sigma       (eq. 32)  =>  sigma = g_y rho_H D^2 / Eo
+ *   Re_Gr = rho_H sqrt(g_y D^3) / mu_H  (eq. 31)  =>  mu_H  = rho_H sqrt(g_y D^3) / Re_Gr
+ *   rho* = rho_H/rho_L, mu* = mu_H/mu_L, nu = mu/rho
+ * out = { g_y, sigma, nu_H, nu_L, rho_L }. */
+int oracle_bubble_params(double Re_Gr, double Eo, double D, double t_ref, double rho_H, double rho_star,
+                         double mu_star, double out[5])
+{
+    if (!out || !(Re_Gr > 0) || !(Eo > 0) || !(D > 0) || !(t_ref > 0) || !(rho_H > 0) || !(rho_star > 0) || !(mu_star > 0))
+        return 1;
+    double gy = D / (t_ref * t_ref);
+    double sigma = gy * rho_H * D * D / Eo;
+    double mu_H = rho_H * sqrt(gy * D * D * D) / Re_Gr;
+    double rho_L = rho_H / rho_star;
+    double mu_L = mu_H / mu_star;
+    out[0] = gy; out[1] = sigma; out[2] = mu_H / rho_H; out[3] = mu_L / rho_L; out[4] = rho_L;
+    return 0;
+}
+
+/* eq. 34: C_D^LBM = 4/3 g_y (rho_H - rho_L) D / (rho_H u_t^2) */
+double oracle_drag_lbm(double gy, double rho_H, double rho_L, double D, double u_t)
+{
+    return (4.0 / 3.0) * gy * (rho_H - rho_L) * D / (rho_H * u_t * u_t);
+}
+
+/* eq. 35: C_D^exp = [ 2.67^(9/10) + (16/Re_Gr)^(9/10) ]^(10/9) */
+double oracle_drag_exp(double Re_Gr)
+{
+    return pow(pow(2.67, 0.9) + pow(16.0 / Re_Gr, 0.9), 10.0 / 9.0);
 }
 
 int oracle_set_threads(int n)
