@@ -33,6 +33,13 @@ def _load():
         lib.oracle_lattice.argtypes = [C.c_int, ip, dp, ip, dp, dp, ip]
         lib.oracle_fd.argtypes = [C.c_void_p, C.c_int, dp, dp, dp]
         lib.oracle_set_threads.argtypes = [C.c_int]
+        lib.oracle_set_variant.argtypes = [C.c_void_p, C.c_uint]
+        lib.oracle_bubble_diag.argtypes = [C.c_void_p, dp]
+        lib.oracle_bubble_params.argtypes = [C.c_double] * 7 + [dp]
+        lib.oracle_drag_lbm.argtypes = [C.c_double] * 5
+        lib.oracle_drag_lbm.restype = C.c_double
+        lib.oracle_drag_exp.argtypes = [C.c_double]
+        lib.oracle_drag_exp.restype = C.c_double
         _lib = lib
     return _lib
 
@@ -62,11 +69,31 @@ def lattice(Q: int):
     return e, w, opp, M, Minv, order
 
 
+VAR_PHASE_SRT = 1
+
+
+def bubble_params(Re_Gr, Eo, D, t_ref, rho_H=1.0, rho_star=1000.0, mu_star=100.0):
+    """eqs. 31-33 solved for the lattice parameters: dict(gy, sigma, nu_H, nu_L, rho_L)."""
+    out = np.zeros(5)
+    rc = _load().oracle_bubble_params(Re_Gr, Eo, D, t_ref, rho_H, rho_star, mu_star, _dp(out))
+    if rc:
+        raise ValueError("bubble_params: all arguments must be positive")
+    return dict(gy=out[0], sigma=out[1], nu_H=out[2], nu_L=out[3], rho_L=out[4])
+
+
+def drag_lbm(gy, rho_H, rho_L, D, u_t):
+    return _load().oracle_drag_lbm(gy, rho_H, rho_L, D, u_t)
+
+
+def drag_exp(Re_Gr):
+    return _load().oracle_drag_exp(Re_Gr)
+
+
 class Oracle:
     """Host-side twin of the acm_* call list."""
 
     def __init__(self, nx, ny, nz, stencil_phase=15, stencil_hydro=19, rho_H=1.0, rho_L=1e-3, sigma=1e-4, xi=5.0,
-                 M=0.02, nu_H=1 / 60, nu_L=1 / 60, gravity=(0.0, 0.0, 0.0), wall_flags=0):
+                 M=0.02, nu_H=1 / 60, nu_L=1 / 60, gravity=(0.0, 0.0, 0.0), wall_flags=0, phase_srt=False):
         self._lib = _load()
         self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
         self.Qh, self.Qg = int(stencil_phase), int(stencil_hydro)
@@ -79,11 +106,13 @@ class Oracle:
         if rc:
             raise ValueError(f"oracle_create failed with code {rc}")
         self._h = h
+        if phase_srt:
+            assert self._lib.oracle_set_variant(h, VAR_PHASE_SRT) == 0
 
     @classmethod
-    def from_params(cls, p):
+    def from_params(cls, p, **kw):
         return cls(p.nx, p.ny, p.nz, p.stencil_phase, p.stencil_hydro, p.rho_H, p.rho_L, p.sigma, p.xi, p.M,
-                   p.nu_H, p.nu_L, p.gravity, p.wall_flags)
+                   p.nu_H, p.nu_L, p.gravity, p.wall_flags, **kw)
 
     def close(self):
         if getattr(self, "_h", None):
@@ -116,6 +145,12 @@ class Oracle:
         if rc:
             raise FloatingPointError("sum(phi) is not finite")
         return t.value
+
+    def bubble_diag(self):
+        """(V, centroid[3] as (x,y,z), velocity[3]) of the light phase, weighted with 1 - phi."""
+        out = np.zeros(7)
+        assert self._lib.oracle_bubble_diag(self._h, _dp(out)) == 0
+        return out[0], out[1:4].copy(), out[4:7].copy()
 
     def get_pdfs(self):
         h = np.empty((self.Qh,) + self.shape)

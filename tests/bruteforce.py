@@ -91,8 +91,9 @@ def laplacian(grid, e, w, C, zyx):
     return 6.0 * sum(w[i] * (C[grid.mirror(zyx, e[i], 1)] - C[zyx]) for i in range(1, len(e)))
 
 
-def step(par, H, G, C, U):
-    """One coupled step.  H[Qh], G[Qg]: lists of numpy (nz,ny,nx) arrays; C: array; U: list of 3 arrays.
+def step(par, H, G, C, U, phase_srt=False):
+    """One coupled step.  phase_srt: Omega^h = omega_phi I (eq. 4 with a single relaxation time).
+     H[Qh], G[Qg]: lists of numpy (nz,ny,nx) arrays; C: array; U: list of 3 arrays.
     Returns new (H, G, C, U) in the oracle's storage convention."""
     import numpy as np
     grid = Grid(par.nx, par.ny, par.nz, par.wall_flags)
@@ -123,7 +124,10 @@ def step(par, H, G, C, U):
         for i in range(Qh):
             coll = 0.0
             for j in range(Qh):
-                om = (1.0 if i == j else 0.0) + (omega - 1.0) * 3.0 * wh[i] * dot(eh[i], eh[j])
+                if phase_srt:
+                    om = omega if i == j else 0.0
+                else:
+                    om = (1.0 if i == j else 0.0) + (omega - 1.0) * 3.0 * wh[i] * dot(eh[i], eh[j])
                 coll += om * d[j]
             Hn[i][zyx] = coll + ht[i] + F[i]
         Cn[zyx] = phin
