@@ -86,8 +86,11 @@ int acm_create(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int ste
  *                     of h and g follows the in-place AA pattern the paper names as the open
  *                     alternative; phi stays double-buffered because its finite-difference
  *                     stencil is non-local.  Same results, same bytes moved per step, half the
- *                     population memory. */
-enum { ACM_OPT_INPLACE = 1, ACM_OPT_ALL = 1 };
+ *                     population memory.
+ *   ACM_OPT_PHASE_SRT single-relaxation-time phase-field collision, Omega^h = omega_phi I: the set-up of
+ *                     the paper's benchmarks ("D3Q15 SRT LB scheme for the interface tracking",
+ *                     P:285) instead of the MRT operator of section 3.1. */
+enum { ACM_OPT_INPLACE = 1, ACM_OPT_PHASE_SRT = 2, ACM_OPT_ALL = 3 };
 size_t acm_workspace_bytes_opt(int nx, int ny, int nz, int stencil_phase, int stencil_hydro, int precision,
                                unsigned options);
 /* acm_create with options; acm_create(...) == acm_create_opt(..., options = 0, ...). */
@@ -114,6 +117,28 @@ int acm_fields(acm_ctx*, void* phi, void* u, void* p);
  * deterministic two-pass block reduction.  Synchronises the stream.  total_host: [host].
  * ACM_EUNSTABLE if the sum is not finite. */
 int acm_phi_mass(acm_ctx*, double* total_host);
+
+/* Rising-bubble diagnostics of section 6.1.  The paper takes "the terminal velocity of
+ * the bubbles" u_t for eq. 34 without saying how it is measured; here (reading A24) the
+ * light phase is weighted with 1 - phi:
+ *   out_host[0]    V   = sum_x (1 - phi)
+ *   out_host[1..3] X_b = sum_x (1 - phi) x_c / V, x_c = cell centre (i + 1/2); plain coordinates
+ *   out_host[4..6] u_b = sum_x (1 - phi) u / V
+ * fp64 accumulation, deterministic two-pass block reduction; synchronises the stream.
+ * ACM_EUNSTABLE if a result is not finite (V = 0 included). */
+int acm_bubble_diag(acm_ctx*, double out_host[7]);
+
+/* Host-only helpers for the set-up and evaluation of section 6.1 (no device work):
+ * acm_bubble_params solves the dimensionless groups for the lattice parameters,
+ *   t_ref = sqrt(D/g_y) (eq. 33), Eo = g_y rho_H D^2/sigma (eq. 32), Re_Gr = rho_H sqrt(g_y D^3)/mu_H
+ *   (eq. 31), rho* = rho_H/rho_L, mu* = mu_H/mu_L, nu = mu/rho;
+ *   out_host = { g_y, sigma, nu_H, nu_L, rho_L }.  ACM_EINVAL unless every argument is > 0.
+ * acm_drag_lbm = 4/3 g_y (rho_H - rho_L) D / (rho_H u_t^2) (eq. 34);
+ * acm_drag_exp = [2.67^(9/10) + (16/Re_Gr)^(9/10)]^(10/9)  (eq. 35). */
+int acm_bubble_params(double Re_Gr, double Eo, double D, double t_ref, double rho_H, double rho_star, double mu_star,
+                      double out_host[5]);
+double acm_drag_lbm(double g_y, double rho_H, double rho_L, double D, double u_t);
+double acm_drag_exp(double Re_Gr);
 
 /* Parity/debug export of the populations in canonical direction order and in the storage
  * convention of the paper's two LB steps: h = post-collision values at their cell (they are

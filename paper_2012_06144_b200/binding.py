@@ -15,10 +15,10 @@ from . import build as _build
 ACM_OK, ACM_EINVAL, ACM_ESTATE, ACM_ECUDA, ACM_EUNSTABLE = 0, 1, 2, 3, 4
 ACM_F64, ACM_F32 = 0, 1
 ACM_WALL_X, ACM_WALL_Y, ACM_WALL_Z = 1, 2, 4
-ACM_OPT_INPLACE = 1
+ACM_OPT_INPLACE, ACM_OPT_PHASE_SRT = 1, 2
 
 EXPORTS = ["acm_workspace_bytes", "acm_workspace_bytes_opt", "acm_create", "acm_create_opt", "acm_init", "acm_step", "acm_fields", "acm_phi_mass", "acm_get_pdfs",
-           "acm_set_pdfs", "acm_run_host", "acm_set_block", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
+           "acm_set_pdfs", "acm_run_host", "acm_bubble_diag", "acm_bubble_params", "acm_drag_lbm", "acm_drag_exp", "acm_set_block", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
 
 _lib = None
 
@@ -59,6 +59,12 @@ def load(build_if_missing: bool = True):
     lib.acm_get_pdfs.argtypes = [vp, vp, vp]
     lib.acm_set_pdfs.argtypes = [vp, vp, vp]
     lib.acm_run_host.argtypes = [vp, vp, vp, i32, vp, vp, vp]
+    lib.acm_bubble_diag.argtypes = [vp, C.POINTER(dbl)]
+    lib.acm_bubble_params.argtypes = [dbl] * 7 + [C.POINTER(dbl)]
+    lib.acm_drag_lbm.argtypes = [dbl] * 5
+    lib.acm_drag_lbm.restype = dbl
+    lib.acm_drag_exp.argtypes = [dbl]
+    lib.acm_drag_exp.restype = dbl
     lib.acm_set_block.argtypes = [vp, i32, i32, i32]
     lib.acm_profile.argtypes = [vp, i32]
     lib.acm_profile_read.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(C.c_longlong)]
@@ -80,12 +86,28 @@ def _ptr(t):
     return None if t is None else C.c_void_p(t.data_ptr())
 
 
+def bubble_params(Re_Gr, Eo, D, t_ref, rho_H=1.0, rho_star=1000.0, mu_star=100.0):
+    """acm_bubble_params: lattice parameters from the dimensionless groups of section 6.1."""
+    lib = load()
+    out = (C.c_double * 5)()
+    _check(lib, lib.acm_bubble_params(Re_Gr, Eo, D, t_ref, rho_H, rho_star, mu_star, out))
+    return dict(gy=out[0], sigma=out[1], nu_H=out[2], nu_L=out[3], rho_L=out[4])
+
+
+def drag_lbm(gy, rho_H, rho_L, D, u_t):
+    return load().acm_drag_lbm(gy, rho_H, rho_L, D, u_t)
+
+
+def drag_exp(Re_Gr):
+    return load().acm_drag_exp(Re_Gr)
+
+
 class ACM:
     """One simulation context: acm_create / acm_init / acm_step / acm_fields / acm_phi_mass."""
 
     def __init__(self, nx, ny, nz, stencil_phase=15, stencil_hydro=19, rho_H=1.0, rho_L=1e-3, sigma=1e-4, xi=5.0,
                  M=0.02, nu_H=1 / 60, nu_L=1 / 60, gravity=(0.0, 0.0, 0.0), wall_flags=0, precision="f64",
-                 device="cuda:0", stream=None, inplace=False):
+                 device="cuda:0", stream=None, inplace=False, phase_srt=False):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2012_06144_b200 needs a CUDA device (no CPU fallback)")
         self._lib = load()
@@ -97,7 +119,7 @@ class ACM:
         self.precision = {"f64": ACM_F64, "f32": ACM_F32}[precision]
         self.dtype = torch.float64 if precision == "f64" else torch.float32
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-        self.options = ACM_OPT_INPLACE if inplace else 0
+        self.options = (ACM_OPT_INPLACE if inplace else 0) | (ACM_OPT_PHASE_SRT if phase_srt else 0)
         nbytes = self._lib.acm_workspace_bytes_opt(self.nx, self.ny, self.nz, self.Qh, self.Qg, self.precision,
                                                    self.options)
         if nbytes == 0:
@@ -155,6 +177,12 @@ class ACM:
         t = C.c_double()
         self._call(self._lib.acm_phi_mass, C.byref(t))
         return t.value
+
+    def bubble_diag(self):
+        """(V, centroid (x,y,z), velocity) of the light phase, weighted with 1 - phi."""
+        out = (C.c_double * 7)()
+        self._call(self._lib.acm_bubble_diag, out)
+        return out[0], tuple(out[1:4]), tuple(out[4:7])
 
     def get_pdfs(self):
         h = torch.empty((self.Qh,) + self.shape, dtype=self.dtype, device=self.device)

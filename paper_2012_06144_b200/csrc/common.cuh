@@ -1,0 +1,231 @@
+// common.cuh -- device building blocks shared by the kernel translation units of libacm:
+// geometry / neighbour indexing, the storage states of a population array and the streaming they
+// imply, the isotropic finite differences of phi, and the argument blocks of the two LB kernels.
+// See DESIGN.md for the data layout.  Shares no code with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstddef>
+#include <cstdint>
+
+#include "../../include/acm.h"
+#include "lattice.cuh"
+
+namespace acm {
+
+// ------------------------------------------------------------------------------------------
+// geometry: neighbour indexing with periodic wrap, wall flags for half-way bounce-back
+// ------------------------------------------------------------------------------------------
+struct Geom {
+    int nx, ny, nz;
+    unsigned walls;
+};
+
+// Per-cell neighbourhood: coordinates of x-1, x, x+1 (periodic wrap; clamped at a wall, which is
+// the mirror ghost phi(x,-1,z) = phi(x,0,z) of the FD stencils) and "beyond a wall" flags.
+struct Nbr {
+    int xs[3];        // x-1, x, x+1
+    int row[3][3];    // [dz+1][dy+1] -> (z'*ny + y')*nx
+    bool wxm, wxp, wym, wyp, wzm, wzp;   // the cell at x-1 / x+1 / ... lies beyond a wall
+
+    template <bool WALLS>
+    __device__ __forceinline__ void setup(const Geom& g, int x, int y, int z)
+    {
+        wxm = wxp = wym = wyp = wzm = wzp = false;
+        int xm = x - 1, xp = x + 1, ym = y - 1, yp = y + 1, zm = z - 1, zp = z + 1;
+        if (xm < 0) { if (WALLS && (g.walls & ACM_WALL_X)) { wxm = true; xm = 0; } else xm = g.nx - 1; }
+        if (xp >= g.nx) { if (WALLS && (g.walls & ACM_WALL_X)) { wxp = true; xp = g.nx - 1; } else xp = 0; }
+        if (ym < 0) { if (WALLS && (g.walls & ACM_WALL_Y)) { wym = true; ym = 0; } else ym = g.ny - 1; }
+        if (yp >= g.ny) { if (WALLS && (g.walls & ACM_WALL_Y)) { wyp = true; yp = g.ny - 1; } else yp = 0; }
+        if (zm < 0) { if (WALLS && (g.walls & ACM_WALL_Z)) { wzm = true; zm = 0; } else zm = g.nz - 1; }
+        if (zp >= g.nz) { if (WALLS && (g.walls & ACM_WALL_Z)) { wzp = true; zp = g.nz - 1; } else zp = 0; }
+        xs[0] = xm; xs[1] = x; xs[2] = xp;
+        const int ys[3] = {ym, y, yp}, zs[3] = {zm, z, zp};
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) row[a][b] = (zs[a] * g.ny + ys[b]) * g.nx;
+    }
+    // index of the cell at offset (dx,dy,dz), each in {-1,0,1}
+    template <int DX, int DY, int DZ>
+    __device__ __forceinline__ int at() const { return row[DZ + 1][DY + 1] + xs[DX + 1]; }
+    // is the cell at offset (dx,dy,dz) beyond a wall?
+    template <int DX, int DY, int DZ, bool WALLS>
+    __device__ __forceinline__ bool beyond() const
+    {
+        if constexpr (!WALLS) return false;
+        bool b = false;
+        if constexpr (DX < 0) b |= wxm;
+        if constexpr (DX > 0) b |= wxp;
+        if constexpr (DY < 0) b |= wym;
+        if constexpr (DY > 0) b |= wyp;
+        if constexpr (DZ < 0) b |= wzm;
+        if constexpr (DZ > 0) b |= wzp;
+        return b;
+    }
+};
+
+// tuning knobs (defaults = the measured best on B200)
+#ifndef ACM_LD
+#define ACM_LD 2
+#endif
+#ifndef ACM_ST
+#define ACM_ST 2
+#endif
+#ifndef ACM_PHASE_MINB
+#define ACM_PHASE_MINB 1
+#endif
+#ifndef ACM_HYDRO_MINB
+#define ACM_HYDRO_MINB 1
+#endif
+#ifndef ACM_MAXT
+#define ACM_MAXT 256
+#endif
+
+// population loads/stores.  Measured on B200 (profiles/r1_variants.md): plain ld/st beat the
+// streaming hints (__ldcs/__stcs) by 5 % on the whole step, so plain is the default.
+template <typename T> __device__ __forceinline__ T ld_stream(const T* p)
+{
+#if ACM_LD == 0
+    return __ldcs(p);
+#elif ACM_LD == 1
+    return __ldg(p);
+#else
+    return *p;
+#endif
+}
+template <typename T> __device__ __forceinline__ void st_stream(T* p, T v)
+{
+#if ACM_ST == 0
+    __stcs(p, v);
+#elif ACM_ST == 1
+    __stcg(p, v);
+#else
+    *p = v;
+#endif
+}
+
+// ------------------------------------------------------------------------------------------
+// Storage states of a population array and the streaming they imply.
+//   ST_POST  (two-grid): slot i at x holds the post-collision f*_i(x); the next step pulls.
+//   ST_IN    (in place): slot i at x holds the incoming (streamed, pre-collision) f_i(x).
+//   ST_SWAP  (in place): slot ibar at x holds the post-collision f*_i(x) (directions swapped).
+// Two-grid update: ST_POST(src) -> ST_POST(dst).  In-place AA pattern (Bailey et al. 2009; the paper
+// names it P:52): even step ST_IN -> ST_SWAP touches only the own cell, odd step ST_SWAP -> ST_IN
+// reads slot ibar at x-e_i and writes slot i at x+e_i -- exactly the locations it read, so one array
+// suffices.  Half-way bounce-back: a population that would come from / go to a cell beyond a wall is
+// taken from / put into the opposite slot of the own cell.
+// ------------------------------------------------------------------------------------------
+enum { ST_POST = 0, ST_IN = 1, ST_SWAP = 2 };
+
+// incoming populations f_i(x) from an array in state STATE
+template <int Q, typename T, bool WALLS, int STATE>
+__device__ __forceinline__ void load_incoming(const T* F, size_t N, const Nbr& nb, T (&f)[Q])
+{
+    using L = Lat<Q>;
+    static_for<0, Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        constexpr int ex = L::ex(i), ey = L::ey(i), ez = L::ez(i), o = L::opp(i);
+        const T* src;
+        if constexpr (STATE == ST_IN) {
+            src = F + (size_t)i * N + nb.template at<0, 0, 0>();
+        } else {
+            constexpr int far = (STATE == ST_POST) ? i : o;      // slot at x - e_i
+            constexpr int own = (STATE == ST_POST) ? o : i;      // slot at x when x - e_i is beyond a wall
+            src = F + (size_t)far * N + nb.template at<-ex, -ey, -ez>();
+            if constexpr (WALLS && i > 0) {
+                if (nb.template beyond<-ex, -ey, -ez, WALLS>()) src = F + (size_t)own * N + nb.template at<0, 0, 0>();
+            }
+        }
+        f[i] = ld_stream(src);
+    });
+}
+
+// address of the post-collision population f*_i(x) in the array the step writes.
+// FROM is the state the step read: ST_POST -> two-grid dst (ST_POST), ST_IN -> ST_SWAP, ST_SWAP -> ST_IN.
+template <int Q, int I, typename T, bool WALLS, int FROM>
+__device__ __forceinline__ T* outgoing_ptr(T* F, size_t N, const Nbr& nb)
+{
+    using L = Lat<Q>;
+    constexpr int ex = L::ex(I), ey = L::ey(I), ez = L::ez(I), o = L::opp(I);
+    if constexpr (FROM == ST_POST) {
+        return F + (size_t)I * N + nb.template at<0, 0, 0>();
+    } else if constexpr (FROM == ST_IN) {
+        return F + (size_t)o * N + nb.template at<0, 0, 0>();
+    } else {
+        T* dst = F + (size_t)I * N + nb.template at<ex, ey, ez>();
+        if constexpr (WALLS && I > 0) {
+            if (nb.template beyond<ex, ey, ez, WALLS>()) dst = F + (size_t)o * N + nb.template at<0, 0, 0>();
+        }
+        return dst;
+    }
+}
+
+// post-collision population f*_i(x) read back from an array in state STATE (export only)
+template <int Q, int I, typename T, int STATE>
+__device__ __forceinline__ T load_post(const T* F, size_t N, const Nbr& nb)
+{
+    using L = Lat<Q>;
+    constexpr int ex = L::ex(I), ey = L::ey(I), ez = L::ez(I), o = L::opp(I);
+    if constexpr (STATE == ST_POST) return F[(size_t)I * N + nb.template at<0, 0, 0>()];
+    else if constexpr (STATE == ST_SWAP) return F[(size_t)o * N + nb.template at<0, 0, 0>()];
+    else {
+        if (nb.template beyond<ex, ey, ez, true>()) return F[(size_t)o * N + nb.template at<0, 0, 0>()];
+        return F[(size_t)I * N + nb.template at<ex, ey, ez>()];
+    }
+}
+
+// Isotropic finite differences of phi on lattice Q (eqs. 23, 24 with c = dx = 1, c_s^2 = 1/3):
+//   grad phi = 3 sum_i w_i e_i phi(x+e_i)      (summed as opposite-pair differences)
+//   lap  phi = 6 sum_i w_i [phi(x+e_i) - phi(x)]
+template <int Q, typename T, bool LAPLACE>
+__device__ __forceinline__ void fd_phi(const T* __restrict__ C, const Nbr& nb, T c0, T& gx, T& gy, T& gz, T& lap)
+{
+    using L = Lat<Q>;
+    T dx[4] = {0, 0, 0, 0}, dy[4] = {0, 0, 0, 0}, dz[4] = {0, 0, 0, 0}, ss[4] = {0, 0, 0, 0};   // per class
+    static_for<1, Q, 2>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        constexpr int ex = L::ex(i), ey = L::ey(i), ez = L::ez(i), c = L::cls(i);
+        const T p = __ldg(C + nb.template at<ex, ey, ez>());
+        const T m = __ldg(C + nb.template at<-ex, -ey, -ez>());
+        const T d = p - m;
+        addsgn<ex>(dx[c], d); addsgn<ey>(dy[c], d); addsgn<ez>(dz[c], d);
+        if constexpr (LAPLACE) ss[c] += p + m;
+    });
+    gx = gy = gz = T(0);
+    T l = T(0), wsum = T(0);
+    static_for<1, 4>([&](auto cc) {
+        constexpr int c = decltype(cc)::value;
+        if constexpr (L::has_cls(c)) {
+            constexpr T w3 = T(3.0 * L::wc(c));
+            gx += w3 * dx[c]; gy += w3 * dy[c]; gz += w3 * dz[c];
+            if constexpr (LAPLACE) l += T(6.0 * L::wc(c)) * ss[c];
+        }
+    });
+    (void)wsum;
+    if constexpr (LAPLACE) lap = l - T(6.0 * (1.0 - L::wc(0))) * c0;   // sum_{i>=1} w_i = 1 - w_0
+}
+
+// ------------------------------------------------------------------------------------------
+// argument blocks of the two LB kernels
+// ------------------------------------------------------------------------------------------
+template <typename T>
+struct PhaseArgs {
+    const T* Hsrc; T* Hdst;
+    const T* Csrc; T* Cdst;
+    const T* U;
+    Geom g;
+    size_t N;
+    T one_minus_omega, inv_xi;
+};
+
+template <typename T>
+struct HydroArgs {
+    const T* Gsrc; T* Gdst;
+    const T* C;      // new phi
+    T* U;
+    Geom g;
+    size_t N;
+    T rho_L, drho, tau_L, dtau, beta4, kappa, gx, gy, gz;
+};
+
+}  // namespace acm

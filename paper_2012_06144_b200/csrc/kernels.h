@@ -1,0 +1,41 @@
+// kernels.h -- host-callable launchers of libacm's CUDA kernels.  Each kernel family lives in its
+// own translation unit (phase_*.cu, hydro_*.cu, aux.cu, ...) so that the library builds in
+// parallel; the launchers dispatch the runtime (stencil, walls, storage state, variant) tuple to
+// the matching template instance and enqueue it on the given stream.  They return the
+// cudaGetLastError() of the launch.
+#pragma once
+#include "common.cuh"
+
+namespace acm {
+
+struct Launch {
+    dim3 grid, block;
+    cudaStream_t stream;
+};
+
+// variants of the phase-field collision (ACM_OPT_PHASE_SRT)
+enum { PHASE_MRT = 0, PHASE_SRT = 1 };
+
+// Fused phase-field LB step (one launch).  state = storage state the kernel reads.
+template <typename T> cudaError_t launch_phase(int Q, bool walls, int state, int collision, const Launch& l, const PhaseArgs<T>& a);
+// Fused hydrodynamic LB step (one launch).
+template <typename T> cudaError_t launch_hydro(int Q, bool walls, int state, const Launch& l, const HydroArgs<T>& a);
+
+// Equilibrium initialiser.
+template <typename T>
+cudaError_t launch_init(int Qh, int Qg, bool inplace, const Launch& l, const T* phi, const T* u, T* H, T* G, T* C, T* U, Geom g, size_t N);
+// Export of a population array stored in `state` in the POST (post-collision at own cell) or
+// incoming convention; optionally the pressure p = c_s^2 rho(phi) sum_i f_i.
+template <typename T>
+cudaError_t launch_export(int Q, int state, bool post, const Launch& l, const T* F, const T* C, T* out, T* p, Geom g, size_t N, T rho_L, T drho);
+// Import: POST convention -> ST_SWAP storage, or incoming convention -> ST_POST storage.
+template <typename T> cudaError_t launch_import(int Q, bool post, const Launch& l, const T* in, T* F, Geom g, size_t N);
+
+// Deterministic two-pass reductions.  `part` holds RED_BLOCKS * width partial sums followed by
+// `width` results.
+constexpr int RED_BLOCKS = 592, RED_THREADS = 256;   // 4 CTAs per SM on 148 SMs
+constexpr int DIAG_WIDTH = 7;                        // V, V*x, V*y, V*z, V*ux, V*uy, V*uz
+template <typename T> cudaError_t launch_sum_phi(cudaStream_t s, const T* C, size_t N, double* part);
+template <typename T> cudaError_t launch_bubble_diag(cudaStream_t s, const T* C, const T* U, Geom g, size_t N, double* part);
+
+}  // namespace acm

@@ -30,7 +30,7 @@ def test_workspace_bytes_and_argument_checks():
     N = 32 ** 3
     b = lib.acm_workspace_bytes(32, 32, 32, 15, 19, 0)
     payload = (2 * (15 + 19) + 2 + 3 + 5) * N * 8
-    assert payload <= b <= payload + 16 * 256 + 8192
+    assert payload <= b <= payload + 16 * 256 + 7 * 593 * 8 + 256      # + reduction scratch
     assert lib.acm_workspace_bytes(32, 32, 32, 15, 19, 1) < b
     assert lib.acm_workspace_bytes(0, 32, 32, 15, 19, 0) == 0
     assert lib.acm_workspace_bytes(32, 32, 32, 13, 19, 0) == 0
@@ -56,3 +56,22 @@ def test_workspace_bytes_and_argument_checks():
     assert lib.acm_step(h, -1) == binding.ACM_EINVAL
     assert lib.acm_launch_count(h) == 0
     lib.acm_destroy(h)
+
+
+def test_host_only_bubble_helpers_match_oracle():
+    """acm_bubble_params / acm_drag_* are host functions (eqs. 31-35): compared with the oracle's
+    own statement of the same equations; argument checks."""
+    from oracle import oracle as om
+    from paper_2012_06144_b200 import binding
+    for Re, Eo, D, t_ref, rs, ms in ((35.0, 30.0, 32.0, 18000.0, 1000.0, 100.0), (50.0, 50.0, 32.0, 18000.0, 1000.0, 100.0),
+                                     (5.0, 1.0, 20.0, 6000.0, 10.0, 1.0)):
+        a = binding.bubble_params(Re, Eo, D, t_ref, 1.0, rs, ms)
+        o = om.bubble_params(Re, Eo, D, t_ref, 1.0, rs, ms)
+        for k in o:
+            assert abs(a[k] - o[k]) <= 1e-15 * abs(o[k]), k
+        assert abs(binding.drag_exp(Re) - om.drag_exp(Re)) < 1e-14
+        assert abs(binding.drag_lbm(a["gy"], 1.0, a["rho_L"], D, 1e-3) / om.drag_lbm(o["gy"], 1.0, o["rho_L"], D, 1e-3) - 1) < 1e-15
+    lib = binding.load()
+    out = (ctypes.c_double * 5)()
+    assert lib.acm_bubble_params(0.0, 1.0, 1.0, 1.0, 1.0, 1.0, 1.0, out) == binding.ACM_EINVAL
+    assert lib.acm_bubble_params(1.0, 1.0, 1.0, 1.0, 1.0, 1.0, 1.0, None) == binding.ACM_EINVAL
