@@ -49,6 +49,9 @@ def workload(config, size=None):
     elif config == 5:
         p, phi, u = inputs.config5() if size is None else inputs.scaled_config3(size, 27, 27)
         name = f"config5: {p.nx}^3 periodic, seeded bubbles + velocity noise, D3Q27+D3Q27"
+    elif config == 6:
+        p, phi, u = inputs.paper_benchmark() if size is None else inputs.paper_benchmark(n=size)
+        name = f"paper benchmark P:283: {p.nx}^3 periodic, one bubble R={p.nx // 4}, D3Q15 SRT + D3Q27 MRT"
     else:
         raise SystemExit(f"unknown config {config}")
     return p, phi, u, name
@@ -120,7 +123,7 @@ def oracle_sample(config, budget_s, steps=None):
     from oracle import Oracle, oracle as om
     cores = om.set_threads(0)
     # calibrate on 24^3
-    p, phi, u, _ = workload(config if config in (1, 3, 5) else 3, size=24)
+    p, phi, u, _ = workload(config if config in (1, 3, 5, 6) else 3, size=24)
     o = Oracle.from_params(p)
     o.init(phi, u)
     o.step(1)
@@ -136,7 +139,7 @@ def oracle_sample(config, budget_s, steps=None):
         n = 64
         while n > 16 and per_cell * n ** 3 * steps > budget_s:
             n -= 8
-    p, phi, u, name = workload(config if config in (1, 3, 5) else 3, size=n)
+    p, phi, u, name = workload(config if config in (1, 3, 5, 6) else 3, size=n)
     o = Oracle.from_params(p)
     o.init(phi, u)
     t = time.perf_counter()
@@ -168,7 +171,8 @@ def workload_name_only(config):
              2: "config2: 128x512x128 rising bubble, walls y, gravity, D3Q15+D3Q19",
              3: "config3: 256^3 periodic, seeded bubbles + velocity noise, D3Q15+D3Q19",
              4: "config4: 512^3 periodic, 512 seeded bubbles, D3Q15+D3Q19",
-             5: "config5: 256^3 periodic, seeded bubbles + velocity noise, D3Q27+D3Q27"}
+             5: "config5: 256^3 periodic, seeded bubbles + velocity noise, D3Q27+D3Q27",
+             6: "paper benchmark P:283: 260^3 periodic, one bubble R=65, D3Q15 SRT + D3Q27 MRT"}
     return None, None, None, names[config]
 
 
@@ -252,9 +256,11 @@ def run_acm(args, rank, local_rank, world):
                     traffic = float(row["dram_bytes_per_launch"])
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+            # BASELINE.md holds the paper's number only for its own benchmark (config 6: 550 MLUPS, P100)
+            "vs_baseline": (value / 550.0 if args.config == 6 and world == 1 and precision == "f64" else None),
             "dtype": precision, "data": "synthetic",
-            "config": {"workload": name, "grid": [p.nx, p.ny, p.nz], "stencils": [p.stencil_phase, p.stencil_hydro], "streaming": "in-place AA" if args.inplace else "two-grid pull",
+            "config": {"workload": name, "grid": [p.nx, p.ny, p.nz], "stencils": [p.stencil_phase, p.stencil_hydro], "phase_collision": "SRT" if p.phase_srt else "MRT", "streaming": "in-place AA" if args.inplace else "two-grid pull",
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": f"inputs larger than L2: {(2 * (p.stencil_phase + p.stencil_hydro) + 5) * N * esz / 1e9:.1f} GB "
                              "of state streamed every step vs 126 MB L2",

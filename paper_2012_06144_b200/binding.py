@@ -138,6 +138,7 @@ class ACM:
 
     @classmethod
     def from_params(cls, p, **kw):
+        kw.setdefault("phase_srt", getattr(p, "phase_srt", False))
         return cls(p.nx, p.ny, p.nz, p.stencil_phase, p.stencil_hydro, p.rho_H, p.rho_L, p.sigma, p.xi, p.M, p.nu_H,
                    p.nu_L, p.gravity, p.wall_flags, **kw)
 

@@ -96,6 +96,17 @@ static int check_launch(acm_ctx* c, const char* what, cudaError_t e, int count =
     return ACM_OK;
 }
 
+// Launch geometry of the two LB kernels: x-rows tiled by the block, or -- when the block is 1-D and
+// nx is not a multiple of it (e.g. the paper's 260^3) -- a linear launch over all cells.
+static bool lb_linear(const acm_ctx* c) { return c->block.y == 1 && c->block.z == 1 && c->nx % (int)c->block.x != 0; }
+
+static Launch lb_launch(const acm_ctx* c)
+{
+    if (lb_linear(c)) return Launch{dim3((unsigned)((c->N + c->block.x - 1) / c->block.x), 1, 1), c->block, c->stream};
+    const dim3 b = c->block;
+    return Launch{dim3((c->nx + b.x - 1) / b.x, (c->ny + b.y - 1) / b.y, (c->nz + b.z - 1) / b.z), b, c->stream};
+}
+
 static dim3 grid_for(const acm_ctx* c, dim3 b)
 {
     return dim3((c->nx + b.x - 1) / b.x, (c->ny + b.y - 1) / b.y, (c->nz + b.z - 1) / b.z);
@@ -116,7 +127,7 @@ static int init_t(acm_ctx* c, const void* phi, const void* u)
     const bool inplace = (c->options & ACM_OPT_INPLACE) != 0;
     T *H = wsp<T>(c, c->offH[0]), *G = wsp<T>(c, c->offG[0]), *C = wsp<T>(c, c->offC[0]), *U = wsp<T>(c, c->offU);
     cudaError_t e = launch_init<T>(c->Qh, c->Qg, inplace, aux_launch(c), (const T*)phi, (const T*)u, H, G, C, U,
-                                   Geom{c->nx, c->ny, c->nz, c->walls}, c->N);
+                                   Geom{c->nx, c->ny, c->nz, c->walls, 0}, c->N);
     if (inplace) { c->stH = ST_SWAP; c->stG = ST_IN; }
     else c->stH = c->stG = ST_POST;
     c->curH = c->curG = c->curC = 0;
@@ -133,12 +144,12 @@ static int launch_phase_step(acm_ctx* c)
     a.Hsrc = wsp<T>(c, c->offH[c->curH]); a.Hdst = wsp<T>(c, c->offH[c->curH ^ 1]);
     a.Csrc = wsp<T>(c, c->offC[c->curC]); a.Cdst = wsp<T>(c, c->offC[c->curC ^ 1]);
     a.U = wsp<T>(c, c->offU);
-    a.g = Geom{c->nx, c->ny, c->nz, c->walls};
+    a.g = Geom{c->nx, c->ny, c->nz, c->walls, lb_linear(c) ? 1 : 0};
     a.N = c->N;
     const double omega = 1.0 / (3.0 * c->M + 0.5);     // tau_phi = M/c_s^2 (eq. 2), shifted by 1/2
     a.one_minus_omega = (T)(1.0 - omega);
     a.inv_xi = (T)(1.0 / c->xi);
-    const Launch l{grid_for(c, c->block), c->block, c->stream};
+    const Launch l = lb_launch(c);
     const int coll = (c->options & ACM_OPT_PHASE_SRT) ? PHASE_SRT : PHASE_MRT;
     cudaError_t e = launch_phase<T>(c->Qh, c->walls != 0, c->stH, coll, l, a);
     c->curH ^= 1; c->curC ^= 1;
@@ -153,13 +164,13 @@ static int launch_hydro_step(acm_ctx* c)
     a.Gsrc = wsp<T>(c, c->offG[c->curG]); a.Gdst = wsp<T>(c, c->offG[c->curG ^ 1]);
     a.C = wsp<T>(c, c->offC[c->curC]);
     a.U = wsp<T>(c, c->offU);
-    a.g = Geom{c->nx, c->ny, c->nz, c->walls};
+    a.g = Geom{c->nx, c->ny, c->nz, c->walls, lb_linear(c) ? 1 : 0};
     a.N = c->N;
     a.rho_L = (T)c->rho_L; a.drho = (T)(c->rho_H - c->rho_L);
     a.tau_L = (T)(3.0 * c->nu_L); a.dtau = (T)(3.0 * c->nu_H - 3.0 * c->nu_L);
     a.beta4 = (T)(4.0 * 12.0 * c->sigma / c->xi); a.kappa = (T)(1.5 * c->sigma * c->xi);
     a.gx = (T)c->grav[0]; a.gy = (T)c->grav[1]; a.gz = (T)c->grav[2];
-    const Launch l{grid_for(c, c->block), c->block, c->stream};
+    const Launch l = lb_launch(c);
     cudaError_t e = launch_hydro<T>(c->Qg, c->walls != 0, c->stG, l, a);
     c->curG ^= 1;
     c->stG = next_state(c->stG);
@@ -194,7 +205,7 @@ template <typename T>
 static int export_g_t(acm_ctx* c, void* g, void* p)      // incoming convention (+ pressure)
 {
     cudaError_t e = launch_export<T>(c->Qg, c->stG, false, aux_launch(c), wsp<T>(c, c->offG[c->curG]), wsp<T>(c, c->offC[c->curC]),
-                                     (T*)g, (T*)p, Geom{c->nx, c->ny, c->nz, c->walls}, c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L));
+                                     (T*)g, (T*)p, Geom{c->nx, c->ny, c->nz, c->walls, 0}, c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L));
     return check_launch(c, "export_kernel", e);
 }
 
@@ -202,7 +213,7 @@ template <typename T>
 static int export_h_t(acm_ctx* c, void* h)               // post-collision convention
 {
     cudaError_t e = launch_export<T>(c->Qh, c->stH, true, aux_launch(c), wsp<T>(c, c->offH[c->curH]), wsp<T>(c, c->offC[c->curC]),
-                                     (T*)h, (T*)nullptr, Geom{c->nx, c->ny, c->nz, c->walls}, c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L));
+                                     (T*)h, (T*)nullptr, Geom{c->nx, c->ny, c->nz, c->walls, 0}, c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L));
     return check_launch(c, "export_kernel", e);
 }
 
@@ -210,7 +221,7 @@ template <typename T>
 static int import_g_t(acm_ctx* c, const void* g)      // incoming convention -> ST_POST storage
 {
     cudaError_t e = launch_import<T>(c->Qg, false, aux_launch(c), (const T*)g, wsp<T>(c, c->offG[c->curG]),
-                                     Geom{c->nx, c->ny, c->nz, c->walls}, c->N);
+                                     Geom{c->nx, c->ny, c->nz, c->walls, 0}, c->N);
     return check_launch(c, "import_kernel", e);
 }
 
@@ -218,7 +229,7 @@ template <typename T>
 static int import_h_t(acm_ctx* c, const void* h)      // post-collision convention -> ST_SWAP storage
 {
     cudaError_t e = launch_import<T>(c->Qh, true, aux_launch(c), (const T*)h, wsp<T>(c, c->offH[c->curH]),
-                                     Geom{c->nx, c->ny, c->nz, c->walls}, c->N);
+                                     Geom{c->nx, c->ny, c->nz, c->walls, 0}, c->N);
     return check_launch(c, "import_kernel", e);
 }
 

@@ -18,7 +18,26 @@ namespace acm {
 struct Geom {
     int nx, ny, nz;
     unsigned walls;
+    int linear;      // 1: the launch is 1-D over all cells (rows not a multiple of the block: no idle tail threads)
 };
+
+// cell of the calling thread: 3-D launch (block tiles of x-rows) or linear launch over the N cells
+__device__ __forceinline__ bool cell_of_thread(const Geom& g, int& x, int& y, int& z)
+{
+    if (g.linear) {
+        const unsigned id = blockIdx.x * blockDim.x + threadIdx.x;
+        if (id >= (unsigned)(g.nx * g.ny * g.nz)) return false;
+        const unsigned t = id / (unsigned)g.nx;
+        x = (int)(id - t * (unsigned)g.nx);
+        z = (int)(t / (unsigned)g.ny);
+        y = (int)(t - (unsigned)z * (unsigned)g.ny);
+        return true;
+    }
+    x = blockIdx.x * blockDim.x + threadIdx.x;
+    y = blockIdx.y * blockDim.y + threadIdx.y;
+    z = blockIdx.z * blockDim.z + threadIdx.z;
+    return x < g.nx && y < g.ny && z < g.nz;
+}
 
 // Per-cell neighbourhood: coordinates of x-1, x, x+1 (periodic wrap; clamped at a wall, which is
 // the mirror ghost phi(x,-1,z) = phi(x,0,z) of the FD stencils) and "beyond a wall" flags.

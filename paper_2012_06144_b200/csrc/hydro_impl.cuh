@@ -15,10 +15,8 @@ namespace acm {
 template <typename T, int Q, bool WALLS, int STATE>
 __global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const HydroArgs<T> a)
 {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x;
-    const int y = blockIdx.y * blockDim.y + threadIdx.y;
-    const int z = blockIdx.z * blockDim.z + threadIdx.z;
-    if (x >= a.g.nx || y >= a.g.ny || z >= a.g.nz) return;
+    int x, y, z;
+    if (!cell_of_thread(a.g, x, y, z)) return;
     Nbr nb;
     nb.setup<WALLS>(a.g, x, y, z);
     const int idx = nb.at<0, 0, 0>();

@@ -52,6 +52,7 @@ class Params:
     nu_L: float = 1.0 / 60.0
     gravity: Tuple[float, float, float] = (0.0, 0.0, 0.0)
     wall_flags: int = 0
+    phase_srt: bool = False      # SRT phase-field collision (the paper's benchmark scheme)
 
     @property
     def shape(self):
@@ -194,6 +195,17 @@ def config4(n: int = 512, count: int = 512):
 
 def config5(n: int = 256, count: int = 64):
     return config3(n=n, count=count, stencil_phase=27, stencil_hydro=27)
+
+
+def paper_benchmark(n: int = 260, R: Optional[float] = None):
+    """The paper's own single-GPU benchmark: n^3 = 260^3 cells, fully periodic, one gas bubble
+    (rho_L = 0.001) of radius 65 in the middle of liquid (rho_H = 1), M = 0.02, xi = 5, sigma = 1e-4,
+    "relaxation time tau = 0.53" (read as the usual tau including the 1/2: nu = (0.53 - 0.5)/3 = 0.01,
+    SURVEY A21), no force, D3Q15 SRT phase field + D3Q27 MRT hydrodynamics."""
+    R = n / 4.0 if R is None else R
+    p = Params(nx=n, ny=n, nz=n, stencil_phase=15, stencil_hydro=27, nu_H=0.01, nu_L=0.01, phase_srt=True)
+    phi = sphere_phi(p, (n / 2.0, n / 2.0, n / 2.0), R, heavy_inside=False)
+    return p, phi, zeros_u(p)
 
 
 def scaled_config3(n: int, stencil_phase: int = 15, stencil_hydro: int = 19):
