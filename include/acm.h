@@ -89,8 +89,14 @@ int acm_create(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int ste
  *                     population memory.
  *   ACM_OPT_PHASE_SRT single-relaxation-time phase-field collision, Omega^h = omega_phi I: the set-up of
  *                     the paper's benchmarks ("D3Q15 SRT LB scheme for the interface tracking",
- *                     P:285) instead of the MRT operator of section 3.1. */
-enum { ACM_OPT_INPLACE = 1, ACM_OPT_PHASE_SRT = 2, ACM_OPT_ALL = 3 };
+ *                     P:285) instead of the MRT operator of section 3.1.
+ *   ACM_OPT_UNFUSED   Algorithm 1 of the paper, kept as a measured comparison for the fusion
+ *                     claim of section 5: the time step as six kernels (stream h, update
+ *                     phi, collide h, stream g, update u, collide g) instead of two.  Same results as
+ *                     the default (Algorithm 2); every population array is read three times and
+ *                     written twice per step.  Needs 3N more workspace (u is double-buffered); cannot
+ *                     be combined with ACM_OPT_INPLACE (ACM_EINVAL). */
+enum { ACM_OPT_INPLACE = 1, ACM_OPT_PHASE_SRT = 2, ACM_OPT_UNFUSED = 4, ACM_OPT_ALL = 7 };
 size_t acm_workspace_bytes_opt(int nx, int ny, int nz, int stencil_phase, int stencil_hydro, int precision,
                                unsigned options);
 /* acm_create with options; acm_create(...) == acm_create_opt(..., options = 0, ...). */

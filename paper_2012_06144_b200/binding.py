@@ -15,7 +15,7 @@ from . import build as _build
 ACM_OK, ACM_EINVAL, ACM_ESTATE, ACM_ECUDA, ACM_EUNSTABLE = 0, 1, 2, 3, 4
 ACM_F64, ACM_F32 = 0, 1
 ACM_WALL_X, ACM_WALL_Y, ACM_WALL_Z = 1, 2, 4
-ACM_OPT_INPLACE, ACM_OPT_PHASE_SRT = 1, 2
+ACM_OPT_INPLACE, ACM_OPT_PHASE_SRT, ACM_OPT_UNFUSED = 1, 2, 4
 
 EXPORTS = ["acm_workspace_bytes", "acm_workspace_bytes_opt", "acm_create", "acm_create_opt", "acm_init", "acm_step", "acm_fields", "acm_phi_mass", "acm_get_pdfs",
            "acm_set_pdfs", "acm_run_host", "acm_bubble_diag", "acm_bubble_params", "acm_drag_lbm", "acm_drag_exp", "acm_set_block", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
@@ -107,7 +107,7 @@ class ACM:
 
     def __init__(self, nx, ny, nz, stencil_phase=15, stencil_hydro=19, rho_H=1.0, rho_L=1e-3, sigma=1e-4, xi=5.0,
                  M=0.02, nu_H=1 / 60, nu_L=1 / 60, gravity=(0.0, 0.0, 0.0), wall_flags=0, precision="f64",
-                 device="cuda:0", stream=None, inplace=False, phase_srt=False):
+                 device="cuda:0", stream=None, inplace=False, phase_srt=False, unfused=False):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2012_06144_b200 needs a CUDA device (no CPU fallback)")
         self._lib = load()
@@ -119,7 +119,7 @@ class ACM:
         self.precision = {"f64": ACM_F64, "f32": ACM_F32}[precision]
         self.dtype = torch.float64 if precision == "f64" else torch.float32
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-        self.options = (ACM_OPT_INPLACE if inplace else 0) | (ACM_OPT_PHASE_SRT if phase_srt else 0)
+        self.options = (ACM_OPT_INPLACE if inplace else 0) | (ACM_OPT_PHASE_SRT if phase_srt else 0) | (ACM_OPT_UNFUSED if unfused else 0)
         nbytes = self._lib.acm_workspace_bytes_opt(self.nx, self.ny, self.nz, self.Qh, self.Qg, self.precision,
                                                    self.options)
         if nbytes == 0:

@@ -43,8 +43,8 @@ struct acm_ctx {
     cudaStream_t stream;
     char* ws;
     // carved workspace (byte offsets)
-    size_t offH[2], offG[2], offC[2], offU, offStage, offRed;
-    int curH, curG, curC;       // which buffer holds the current state
+    size_t offH[2], offG[2], offC[2], offU[2], offStage, offRed;
+    int curH, curG, curC, curU;       // which buffer holds the current state
     unsigned options;           // ACM_OPT_*
     int stH, stG;               // storage state of the current H / G buffer (ST_POST | ST_IN | ST_SWAP)
     bool initialised;
@@ -62,12 +62,13 @@ static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 static bool valid_stencil(int q) { return q == 15 || q == 19 || q == 27; }
 
 struct Layout {
-    size_t offH[2], offG[2], offC[2], offU, offStage, offRed, total;
+    size_t offH[2], offG[2], offC[2], offU[2], offStage, offRed, total;
 };
 
 static bool make_layout(int nx, int ny, int nz, int Qh, int Qg, int precision, unsigned options, Layout* L)
 {
     if (options & ~(unsigned)ACM_OPT_ALL) return false;
+    if ((options & ACM_OPT_UNFUSED) && (options & ACM_OPT_INPLACE)) return false;   // Algorithm 1 is a two-grid scheme
     const int grids = (options & ACM_OPT_INPLACE) ? 1 : 2;
     if (nx <= 0 || ny <= 0 || nz <= 0 || !valid_stencil(Qh) || !valid_stencil(Qg)) return false;
     if (precision != ACM_F64 && precision != ACM_F32) return false;
@@ -79,7 +80,8 @@ static bool make_layout(int nx, int ny, int nz, int Qh, int Qg, int precision, u
     for (int b = 0; b < grids; ++b) { L->offG[b] = o; o = align256(o + (size_t)Qg * N * e); }
     if (grids == 1) { L->offH[1] = L->offH[0]; L->offG[1] = L->offG[0]; }
     for (int b = 0; b < 2; ++b) { L->offC[b] = o; o = align256(o + N * e); }
-    L->offU = o; o = align256(o + 3 * N * e);
+    L->offU[0] = L->offU[1] = o; o = align256(o + 3 * N * e);
+    if (options & ACM_OPT_UNFUSED) { L->offU[1] = o; o = align256(o + 3 * N * e); }   // u double-buffered (unfused_impl.cuh)
     L->offStage = o; o = align256(o + 5 * N * e);
     L->offRed = o; o = align256(o + (size_t)DIAG_WIDTH * (RED_BLOCKS + 1) * sizeof(double));
     L->total = o;
@@ -125,12 +127,12 @@ template <typename T>
 static int init_t(acm_ctx* c, const void* phi, const void* u)
 {
     const bool inplace = (c->options & ACM_OPT_INPLACE) != 0;
-    T *H = wsp<T>(c, c->offH[0]), *G = wsp<T>(c, c->offG[0]), *C = wsp<T>(c, c->offC[0]), *U = wsp<T>(c, c->offU);
+    T *H = wsp<T>(c, c->offH[0]), *G = wsp<T>(c, c->offG[0]), *C = wsp<T>(c, c->offC[0]), *U = wsp<T>(c, c->offU[0]);
     cudaError_t e = launch_init<T>(c->Qh, c->Qg, inplace, aux_launch(c), (const T*)phi, (const T*)u, H, G, C, U,
                                    Geom{c->nx, c->ny, c->nz, c->walls, 0}, c->N);
     if (inplace) { c->stH = ST_SWAP; c->stG = ST_IN; }
     else c->stH = c->stG = ST_POST;
-    c->curH = c->curG = c->curC = 0;
+    c->curH = c->curG = c->curC = c->curU = 0;
     return check_launch(c, "init_kernel", e);
 }
 
@@ -143,7 +145,7 @@ static int launch_phase_step(acm_ctx* c)
     PhaseArgs<T> a;
     a.Hsrc = wsp<T>(c, c->offH[c->curH]); a.Hdst = wsp<T>(c, c->offH[c->curH ^ 1]);
     a.Csrc = wsp<T>(c, c->offC[c->curC]); a.Cdst = wsp<T>(c, c->offC[c->curC ^ 1]);
-    a.U = wsp<T>(c, c->offU);
+    a.U = wsp<T>(c, c->offU[c->curU]);
     a.g = Geom{c->nx, c->ny, c->nz, c->walls, lb_linear(c) ? 1 : 0};
     a.N = c->N;
     const double omega = 1.0 / (3.0 * c->M + 0.5);     // tau_phi = M/c_s^2 (eq. 2), shifted by 1/2
@@ -151,10 +153,12 @@ static int launch_phase_step(acm_ctx* c)
     a.inv_xi = (T)(1.0 / c->xi);
     const Launch l = lb_launch(c);
     const int coll = (c->options & ACM_OPT_PHASE_SRT) ? PHASE_SRT : PHASE_MRT;
-    cudaError_t e = launch_phase<T>(c->Qh, c->walls != 0, c->stH, coll, l, a);
+    const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
+    cudaError_t e = unfused ? launch_unfused_phase<T>(c->Qh, c->walls != 0, coll, l, a)
+                            : launch_phase<T>(c->Qh, c->walls != 0, c->stH, coll, l, a);
     c->curH ^= 1; c->curC ^= 1;
     c->stH = next_state(c->stH);
-    return check_launch(c, "phase_kernel", e);
+    return check_launch(c, unfused ? "stream_h/phi/collide_h kernels" : "phase_kernel", e, unfused ? 3 : 1);
 }
 
 template <typename T>
@@ -163,7 +167,7 @@ static int launch_hydro_step(acm_ctx* c)
     HydroArgs<T> a;
     a.Gsrc = wsp<T>(c, c->offG[c->curG]); a.Gdst = wsp<T>(c, c->offG[c->curG ^ 1]);
     a.C = wsp<T>(c, c->offC[c->curC]);
-    a.U = wsp<T>(c, c->offU);
+    a.U = wsp<T>(c, c->offU[c->curU]);
     a.g = Geom{c->nx, c->ny, c->nz, c->walls, lb_linear(c) ? 1 : 0};
     a.N = c->N;
     a.rho_L = (T)c->rho_L; a.drho = (T)(c->rho_H - c->rho_L);
@@ -171,10 +175,17 @@ static int launch_hydro_step(acm_ctx* c)
     a.beta4 = (T)(4.0 * 12.0 * c->sigma / c->xi); a.kappa = (T)(1.5 * c->sigma * c->xi);
     a.gx = (T)c->grav[0]; a.gy = (T)c->grav[1]; a.gz = (T)c->grav[2];
     const Launch l = lb_launch(c);
-    cudaError_t e = launch_hydro<T>(c->Qg, c->walls != 0, c->stG, l, a);
+    const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
+    cudaError_t e;
+    if (unfused) {
+        e = launch_unfused_hydro<T>(c->Qg, c->walls != 0, l, a, wsp<T>(c, c->offU[c->curU]), wsp<T>(c, c->offU[c->curU ^ 1]));
+        c->curU ^= 1;
+    } else {
+        e = launch_hydro<T>(c->Qg, c->walls != 0, c->stG, l, a);
+    }
     c->curG ^= 1;
     c->stG = next_state(c->stG);
-    return check_launch(c, "hydro_kernel", e);
+    return check_launch(c, unfused ? "stream_g/velocity/collide_g kernels" : "hydro_kernel", e, unfused ? 3 : 1);
 }
 
 static void prof_mark(acm_ctx* c)
@@ -299,8 +310,8 @@ int acm_create_opt(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int
     c->stream = (cudaStream_t)cuda_stream;
     c->ws = (char*)workspace;
     for (int b = 0; b < 2; ++b) { c->offH[b] = L.offH[b]; c->offG[b] = L.offG[b]; c->offC[b] = L.offC[b]; }
-    c->offU = L.offU; c->offStage = L.offStage; c->offRed = L.offRed;
-    c->curH = c->curG = c->curC = 0;
+    c->offU[0] = L.offU[0]; c->offU[1] = L.offU[1]; c->offStage = L.offStage; c->offRed = L.offRed;
+    c->curH = c->curG = c->curC = c->curU = 0;
     c->options = options;
     c->stH = c->stG = ST_POST;
     c->initialised = false;
@@ -394,7 +405,7 @@ int acm_fields(acm_ctx* c, void* phi, void* u, void* p)
     if (!c->initialised) return fail(ACM_ESTATE, "acm_fields: call acm_init first");
     int rc = ACM_OK;
     if (phi) rc = copy_async(c, phi, c->ws + c->offC[c->curC], c->N * c->esz, cudaMemcpyDeviceToDevice, "acm_fields(phi)");
-    if (!rc && u) rc = copy_async(c, u, c->ws + c->offU, 3 * c->N * c->esz, cudaMemcpyDeviceToDevice, "acm_fields(u)");
+    if (!rc && u) rc = copy_async(c, u, c->ws + c->offU[c->curU], 3 * c->N * c->esz, cudaMemcpyDeviceToDevice, "acm_fields(u)");
     if (!rc && p) rc = c->precision == ACM_F64 ? export_g_t<double>(c, nullptr, p) : export_g_t<float>(c, nullptr, p);
     return rc;
 }
@@ -425,8 +436,8 @@ int acm_bubble_diag(acm_ctx* c, double out_host[7])
     double* part = wsp<double>(c, c->offRed);
     const Geom g{c->nx, c->ny, c->nz, c->walls};
     cudaError_t le = c->precision == ACM_F64
-                         ? launch_bubble_diag<double>(c->stream, wsp<double>(c, c->offC[c->curC]), wsp<double>(c, c->offU), g, c->N, part)
-                         : launch_bubble_diag<float>(c->stream, wsp<float>(c, c->offC[c->curC]), wsp<float>(c, c->offU), g, c->N, part);
+                         ? launch_bubble_diag<double>(c->stream, wsp<double>(c, c->offC[c->curC]), wsp<double>(c, c->offU[c->curU]), g, c->N, part)
+                         : launch_bubble_diag<float>(c->stream, wsp<float>(c, c->offC[c->curC]), wsp<float>(c, c->offU[c->curU]), g, c->N, part);
     int rc = check_launch(c, "bubble_diag", le, 2);
     if (rc) return rc;
     double sums[DIAG_WIDTH];
@@ -512,7 +523,7 @@ int acm_run_host(acm_ctx* c, const void* phi_host, const void* u_host, int n, vo
     if (!rc) rc = acm_step(c, n);
     if (!rc && p_out_host) rc = acm_fields(c, nullptr, nullptr, st + 4 * fb);
     if (!rc && phi_out_host) rc = copy_async(c, phi_out_host, c->ws + c->offC[c->curC], fb, cudaMemcpyDeviceToHost, "acm_run_host(d2h phi)");
-    if (!rc && u_out_host) rc = copy_async(c, u_out_host, c->ws + c->offU, 3 * fb, cudaMemcpyDeviceToHost, "acm_run_host(d2h u)");
+    if (!rc && u_out_host) rc = copy_async(c, u_out_host, c->ws + c->offU[c->curU], 3 * fb, cudaMemcpyDeviceToHost, "acm_run_host(d2h u)");
     if (!rc && p_out_host) rc = copy_async(c, p_out_host, st + 4 * fb, fb, cudaMemcpyDeviceToHost, "acm_run_host(d2h p)");
     if (rc) return rc;
     cudaError_t e = cudaStreamSynchronize(c->stream);

@@ -136,6 +136,9 @@ template <typename T> __device__ __forceinline__ void st_stream(T* p, T v)
 // ------------------------------------------------------------------------------------------
 enum { ST_POST = 0, ST_IN = 1, ST_SWAP = 2 };
 
+// variants of the phase-field collision (ACM_OPT_PHASE_SRT)
+enum { PHASE_MRT = 0, PHASE_SRT = 1 };
+
 // incoming populations f_i(x) from an array in state STATE
 template <int Q, typename T, bool WALLS, int STATE>
 __device__ __forceinline__ void load_incoming(const T* F, size_t N, const Nbr& nb, T (&f)[Q])

@@ -13,13 +13,15 @@ struct Launch {
     cudaStream_t stream;
 };
 
-// variants of the phase-field collision (ACM_OPT_PHASE_SRT)
-enum { PHASE_MRT = 0, PHASE_SRT = 1 };
-
 // Fused phase-field LB step (one launch).  state = storage state the kernel reads.
 template <typename T> cudaError_t launch_phase(int Q, bool walls, int state, int collision, const Launch& l, const PhaseArgs<T>& a);
 // Fused hydrodynamic LB step (one launch).
 template <typename T> cudaError_t launch_hydro(int Q, bool walls, int state, const Launch& l, const HydroArgs<T>& a);
+
+// Algorithm 1, three launches each: stream h -> update phi -> collide h, and
+// stream g -> update u (Uold -> Unew) -> collide g.  Two-grid storage only (a.Hsrc/a.Gsrc in ST_POST).
+template <typename T> cudaError_t launch_unfused_phase(int Q, bool walls, int collision, const Launch& l, const PhaseArgs<T>& a);
+template <typename T> cudaError_t launch_unfused_hydro(int Q, bool walls, const Launch& l, const HydroArgs<T>& a, const T* Uold, T* Unew);
 
 // Equilibrium initialiser.
 template <typename T>

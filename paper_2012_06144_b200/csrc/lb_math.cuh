@@ -1,0 +1,139 @@
+// lb_math.cuh -- the per-cell arithmetic of the two LB steps as device functions, shared by the fused
+// kernels (phase_impl.cuh, hydro_impl.cuh: Algorithm 2) and the unfused six-kernel pipeline
+// (unfused_impl.cuh: Algorithm 1), so that both evaluate exactly the same expressions.
+#pragma once
+#include "common.cuh"
+
+namespace acm {
+
+// Phase-field collision at one cell (eqs. 4-6): from the streamed populations h (their
+// moments m, phi = m.m0), the OLD phi at the cell (c0) and its gradient (gx,gy,gz), and u, emit the
+// post-collision populations through store(ic, value).
+template <typename T, int Q, int COLL, typename Store>
+__device__ __forceinline__ void phase_collide(const T (&h)[Q], const Moments<Q, T, false>& m, T c0, T gx, T gy, T gz, T ux, T uy,
+                                              T uz, T one_minus_omega, T inv_xi, Store&& store)
+{
+    const T phi = m.m0;
+    // interface normal (n = 0 where grad phi vanishes exactly) and theta = (1 - 4 (phi-1/2)^2)/xi
+    const T g2 = gx * gx + gy * gy + gz * gz;
+    const T inv = (g2 > T(0)) ? T(1) / sqrt(g2) : T(0);
+    const T dc = c0 - T(0.5);
+    const T theta = (T(1) - T(4) * dc * dc) * inv_xi;
+    const T tnx = theta * inv * gx, tny = theta * inv * gy, tnz = theta * inv * gz;   // theta * n
+
+    // closed form of the collision: h*_i = w_i [A + e_i.b + e_i e_i : T] (+ keep * h_i for SRT)
+    T A, bx, by, bz, Ts, keep;
+    if constexpr (COLL == PHASE_MRT) {
+        // first-order moments relaxed with omega_phi, all others with 1 (A3):
+        // with d = j - phi u + (theta/6) n:  h*_i = phi Gamma_i(u) + F_i/2 + (1-omega) 3 w_i e_i.d
+        const T k = T(3) * one_minus_omega;
+        const T sixth = T(1.0 / 6.0);
+        const T dxm = m.jx - phi * ux + sixth * tnx;
+        const T dym = m.jy - phi * uy + sixth * tny;
+        const T dzm = m.jz - phi * uz + sixth * tnz;
+        const T p3 = T(3) * phi;
+        A = phi * (T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz));
+        bx = p3 * ux + T(0.5) * tnx + k * dxm;
+        by = p3 * uy + T(0.5) * tny + k * dym;
+        bz = p3 * uz + T(0.5) * tnz + k * dzm;
+        Ts = T(4.5) * phi;
+        keep = T(0);
+    } else {
+        // single relaxation time (A23): h*_i = (1-omega) h_i + omega phi Gamma_i(u) + (1-omega/2) F_i
+        const T omega = T(1) - one_minus_omega;
+        const T op = omega * phi, fh = T(1) - T(0.5) * omega;
+        A = op * (T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz));
+        bx = T(3) * op * ux + fh * tnx;
+        by = T(3) * op * uy + fh * tny;
+        bz = T(3) * op * uz + fh * tnz;
+        Ts = T(4.5) * op;
+        keep = one_minus_omega;
+    }
+    auto post = [&](auto ic, T v) -> T {
+        if constexpr (COLL == PHASE_SRT) return v + keep * h[decltype(ic)::value];
+        else return v;
+    };
+    if constexpr (sizeof(T) == 8) {
+        emit_populations<Q, T>(A, bx, by, bz, Ts * ux * ux, Ts * uy * uy, Ts * uz * uz, Ts * ux * uy, Ts * ux * uz,
+                               Ts * uy * uz, [&](auto ic, T v) {
+                                   store(ic, post(ic, v));
+                               });
+    } else {
+        // fp32 instance (reading A22): the rest population is set by subtraction,
+        // h*_0 = phi_new - sum_{i>=1} h*_i, so that the collision conserves phi exactly in fp32.
+        T rest = phi;
+        emit_populations<Q, T>(A, bx, by, bz, Ts * ux * ux, Ts * uy * uy, Ts * uz * uz, Ts * ux * uy, Ts * ux * uz,
+                               Ts * uy * uz, [&](auto ic, T v) {
+                                   constexpr int i = decltype(ic)::value;
+                                   if constexpr (i > 0) {
+                                       const T o = post(ic, v);
+                                       rest -= o;
+                                       store(ic, o);
+                                   }
+                               });
+        store(std::integral_constant<int, 0>{}, rest);
+    }
+}
+
+// Hydrodynamic forces and velocity at one cell (eqs. 8, 13-22, 30): from the moments m of the incoming
+// populations g, the NEW phi at the cell (c0) with its gradient and Laplacian, and the velocity of the
+// previous step (uo), compute u_new = j + F/(2 rho) and keep what the collision needs.
+template <typename T>
+struct HydroCell {
+    T ux, uy, uz;      // u_new, eq. 22
+    T hx, hy, hz;      // F/(2 rho)
+    T s_nu;            // eq. 21
+    T Sxx, Syy, Szz;   // P_aa - p*/3
+};
+
+template <typename T, int Q>
+__device__ __forceinline__ HydroCell<T> hydro_velocity(const Moments<Q, T, true>& m, T c0, T gpx, T gpy, T gpz, T lap, T uox, T uoy,
+                                                       T uoz, const HydroArgs<T>& a)
+{
+    const T pstar = m.m0;
+    const T p3 = pstar * T(1.0 / 3.0);
+
+    const T rho = a.rho_L + c0 * a.drho;                  // eq. 8 (phi_L = 0)
+    const T inv_rho = T(1) / rho;
+    const T tau = a.tau_L + c0 * a.dtau;                  // eq. 20
+    const T s_nu = T(1) / (tau + T(0.5));                 // eq. 21
+    const T mu = a.beta4 * c0 * (c0 - T(1)) * (c0 - T(0.5)) - a.kappa * lap;   // eq. 17
+    const T grx = a.drho * gpx, gry = a.drho * gpy, grz = a.drho * gpz;
+
+    // deviatoric second moment without the velocity part
+    const T Sxx = m.Pxx - p3, Syy = m.Pyy - p3, Szz = m.Pzz - p3;
+    // viscous force with the velocity of the previous step (eq. 18)
+    const T ts = -tau * s_nu;
+    const T oxx = Sxx - uox * uox, oyy = Syy - uoy * uoy, ozz = Szz - uoz * uoz;
+    const T oxy = m.Pxy - uox * uoy, oxz = m.Pxz - uox * uoz, oyz = m.Pyz - uoy * uoz;
+    const T Fx = mu * gpx - p3 * grx + ts * (oxx * grx + oxy * gry + oxz * grz) + rho * a.gx;
+    const T Fy = mu * gpy - p3 * gry + ts * (oxy * grx + oyy * gry + oyz * grz) + rho * a.gy;
+    const T Fz = mu * gpz - p3 * grz + ts * (oxz * grx + oyz * gry + ozz * grz) + rho * a.gz;
+    // velocity, eq. 22
+    const T hx = T(0.5) * Fx * inv_rho, hy = T(0.5) * Fy * inv_rho, hz = T(0.5) * Fz * inv_rho;
+    const T ux = m.jx + hx, uy = m.jy + hy, uz = m.jz + hz;
+    return HydroCell<T>{ux, uy, uz, hx, hy, hz, s_nu, Sxx, Syy, Szz};
+}
+
+// Hydrodynamic collision at one cell (eqs. 10-12, 25 in closed form): emits the
+// post-collision populations through store(ic, value).
+template <typename T, int Q, typename Store>
+__device__ __forceinline__ void hydro_collide(const Moments<Q, T, true>& m, const HydroCell<T>& hc, Store&& store)
+{
+    const T pstar = m.m0;
+    const T ux = hc.ux, uy = hc.uy, uz = hc.uz, hx = hc.hx, hy = hc.hy, hz = hc.hz, s_nu = hc.s_nu;
+    const T Sxx = hc.Sxx, Syy = hc.Syy, Szz = hc.Szz;
+    // collision
+    const T om = T(1) - s_nu;
+    const T nxx = Sxx - ux * ux, nyy = Syy - uy * uy, nzz = Szz - uz * uz;
+    const T k45 = T(4.5) * om, s45 = T(4.5);
+    const T Txx = s45 * ux * ux + k45 * nxx, Tyy = s45 * uy * uy + k45 * nyy, Tzz = s45 * uz * uz + k45 * nzz;
+    const T Txy = s45 * ux * uy + k45 * (m.Pxy - ux * uy);
+    const T Txz = s45 * ux * uz + k45 * (m.Pxz - ux * uz);
+    const T Tyz = s45 * uy * uz + k45 * (m.Pyz - uy * uz);
+    const T A = pstar - T(1.5) * (ux * ux + uy * uy + uz * uz) - T(1.5) * om * (nxx + nyy + nzz);
+    const T bx = T(3) * (ux + hx), by = T(3) * (uy + hy), bz = T(3) * (uz + hz);
+    emit_populations<Q, T>(A, bx, by, bz, Txx, Tyy, Tzz, Txy, Txz, Tyz, store);
+}
+
+}  // namespace acm

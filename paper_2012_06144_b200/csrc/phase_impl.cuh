@@ -1,6 +1,7 @@
 // phase_impl.cuh -- fused phase-field LB kernel and its launcher, instantiated for one element
 // type per translation unit (phase_f64.cu, phase_f32.cu define ACM_T and include this file).
 #include "kernels.h"
+#include "lb_math.cuh"
 
 namespace acm {
 
@@ -31,65 +32,9 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const P
     m.compute(h);
     const T phi = m.m0;
 
-    // interface normal (n = 0 where grad phi vanishes exactly) and theta = (1 - 4 (phi-1/2)^2)/xi
-    const T g2 = gx * gx + gy * gy + gz * gz;
-    const T inv = (g2 > T(0)) ? T(1) / sqrt(g2) : T(0);
-    const T dc = c0 - T(0.5);
-    const T theta = (T(1) - T(4) * dc * dc) * a.inv_xi;
-    const T tnx = theta * inv * gx, tny = theta * inv * gy, tnz = theta * inv * gz;   // theta * n
-
-    // closed form of the collision: h*_i = w_i [A + e_i.b + e_i e_i : T] (+ keep * h_i for SRT)
-    T A, bx, by, bz, Ts, keep;
-    if constexpr (COLL == PHASE_MRT) {
-        // first-order moments relaxed with omega_phi, all others with 1 (A3):
-        // with d = j - phi u + (theta/6) n:  h*_i = phi Gamma_i(u) + F_i/2 + (1-omega) 3 w_i e_i.d
-        const T k = T(3) * a.one_minus_omega;
-        const T sixth = T(1.0 / 6.0);
-        const T dxm = m.jx - phi * ux + sixth * tnx;
-        const T dym = m.jy - phi * uy + sixth * tny;
-        const T dzm = m.jz - phi * uz + sixth * tnz;
-        const T p3 = T(3) * phi;
-        A = phi * (T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz));
-        bx = p3 * ux + T(0.5) * tnx + k * dxm;
-        by = p3 * uy + T(0.5) * tny + k * dym;
-        bz = p3 * uz + T(0.5) * tnz + k * dzm;
-        Ts = T(4.5) * phi;
-        keep = T(0);
-    } else {
-        // single relaxation time (A23): h*_i = (1-omega) h_i + omega phi Gamma_i(u) + (1-omega/2) F_i
-        const T omega = T(1) - a.one_minus_omega;
-        const T op = omega * phi, fh = T(1) - T(0.5) * omega;
-        A = op * (T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz));
-        bx = T(3) * op * ux + fh * tnx;
-        by = T(3) * op * uy + fh * tny;
-        bz = T(3) * op * uz + fh * tnz;
-        Ts = T(4.5) * op;
-        keep = a.one_minus_omega;
-    }
-    auto post = [&](auto ic, T v) -> T {
-        if constexpr (COLL == PHASE_SRT) return v + keep * h[decltype(ic)::value];
-        else return v;
-    };
-    if constexpr (sizeof(T) == 8) {
-        emit_populations<Q, T>(A, bx, by, bz, Ts * ux * ux, Ts * uy * uy, Ts * uz * uz, Ts * ux * uy, Ts * ux * uz,
-                               Ts * uy * uz, [&](auto ic, T v) {
-                                   st_stream(outgoing_ptr<Q, decltype(ic)::value, T, WALLS, STATE>(a.Hdst, N, nb), post(ic, v));
-                               });
-    } else {
-        // fp32 instance (reading A22): the rest population is set by subtraction,
-        // h*_0 = phi_new - sum_{i>=1} h*_i, so that the collision conserves phi exactly in fp32.
-        T rest = phi;
-        emit_populations<Q, T>(A, bx, by, bz, Ts * ux * ux, Ts * uy * uy, Ts * uz * uz, Ts * ux * uy, Ts * ux * uz,
-                               Ts * uy * uz, [&](auto ic, T v) {
-                                   constexpr int i = decltype(ic)::value;
-                                   if constexpr (i > 0) {
-                                       const T o = post(ic, v);
-                                       rest -= o;
-                                       st_stream(outgoing_ptr<Q, i, T, WALLS, STATE>(a.Hdst, N, nb), o);
-                                   }
-                               });
-        st_stream(outgoing_ptr<Q, 0, T, WALLS, STATE>(a.Hdst, N, nb), rest);
-    }
+    phase_collide<T, Q, COLL>(h, m, c0, gx, gy, gz, ux, uy, uz, a.one_minus_omega, a.inv_xi, [&](auto ic, T v) {
+        st_stream(outgoing_ptr<Q, decltype(ic)::value, T, WALLS, STATE>(a.Hdst, N, nb), v);
+    });
     a.Cdst[idx] = phi;
 }
 
