@@ -146,6 +146,66 @@ int acm_bubble_params(double Re_Gr, double Eo, double D, double t_ref, double rh
 double acm_drag_lbm(double g_y, double rho_H, double rho_L, double D, double u_t);
 double acm_drag_exp(double Re_Gr);
 
+/* Un-normalised sums behind acm_bubble_diag: { sum w, sum w x_c, sum w y_c, sum w z_c, sum w u_x, sum w u_y,
+ * sum w u_z } with w = 1 - phi over the cells this context owns (z_c in global coordinates for a slab), so that
+ * the slabs of a decomposed domain can be added up before normalising. */
+int acm_bubble_sums(acm_ctx*, double out_host[7]);
+
+/* ---- Slab decomposition along z (the paper's block decomposition with one ghost layer,
+ * P:203, and its inner / outer split for communication hiding, Alg. 2 and Fig. 3) -------
+ *
+ * The global grid nx x ny x nz_global is cut into `nranks` slabs of consecutive z planes, one context (one
+ * GPU, one process) each.  A slab stores its owned planes plus ONE ghost plane below and above:
+ * every field array handed to or returned by a slab context has nz_local + 2 planes, plane 0 and plane
+ * nz_local + 1 being the ghosts (arrays returned by the library leave them unspecified).
+ * Periodicity / walls in z apply to the global domain; x and y are handled as before.
+ *
+ * The library does not communicate.  It tells the caller which byte ranges of the workspace have to travel
+ * (acm_halo_plan) and lets it launch the two LB kernels on sub-ranges of planes, so that the caller
+ * (paper_2012_06144_b200/slab.py: torch.distributed over NCCL/NVLink) overlaps the exchange with the kernels:
+ *
+ *   per step:  acm_phase_launch(0, nzl); acm_phase_commit            needs: h and phi ghosts
+ *              exchange ACM_HALO_PHI (new phi) and ACM_HALO_H        (h is only needed by the NEXT phase step)
+ *              acm_hydro_launch(1, nzl-1)                            inner planes: no ghost is read
+ *              wait for ACM_HALO_PHI (and the g ghosts of the previous step)
+ *              acm_hydro_launch(0, 1); acm_hydro_launch(nzl-1, nzl); acm_hydro_commit
+ *              exchange ACM_HALO_G                                   (only needed by the NEXT hydrodynamic step)
+ *
+ * ACM_OPT_INPLACE and ACM_OPT_UNFUSED are not available for slabs; acm_step and acm_run_host return ACM_ESTATE. */
+
+/* Planes [*z_begin, *z_begin + *z_count) of the global grid owned by `rank` (the first nz_global % nranks
+ * slabs get one plane more).  Host only.  ACM_EINVAL unless 1 <= nranks <= nz_global, 0 <= rank < nranks. */
+int acm_slab_range(int nz_global, int rank, int nranks, int* z_begin, int* z_count);
+size_t acm_workspace_bytes_slab(int nx, int ny, int nz_global, int stencil_phase, int stencil_hydro, int precision,
+                                int rank, int nranks);
+/* acm_create_opt for the slab `rank` of `nranks`; all other arguments describe the GLOBAL problem. */
+int acm_create_slab(acm_ctx** out, int nx, int ny, int nz_global, int stencil_phase, int stencil_hydro,
+                    double rho_H, double rho_L, double sigma, double xi, double M, double nu_H, double nu_L,
+                    const double gravity[3], unsigned wall_flags, int precision, unsigned options,
+                    int rank, int nranks, void* workspace, void* cuda_stream);
+/* info = { rank, nranks, first owned global plane, owned planes, allocated planes, has ghost planes (0/1) }. */
+int acm_slab_info(const acm_ctx*, int info[6]);
+
+/* What has to cross the z face `side` (0 = low z, 1 = high z) of this slab for the CURRENT buffers:
+ *   ACM_HALO_H    phase populations: the e_z != 0 directions only (5 planes for D3Q15/19, 9 for D3Q27)
+ *   ACM_HALO_G    hydrodynamic populations, likewise
+ *   ACM_HALO_PHI  the phase field (1 plane)
+ * recv = 0: the planes to SEND (this slab's outermost owned plane at that face);
+ * recv = 1: the planes to RECEIVE INTO (this slab's ghost plane at that face).
+ * Writes up to max_chunks (offset, bytes) pairs, offsets in bytes from the workspace base, and returns their
+ * number, or -(error code).  The k-th chunk sent through a low face matches the k-th chunk received at the
+ * neighbour's high face and vice versa.  Host only (valid without a GPU). */
+enum { ACM_HALO_H = 0, ACM_HALO_G = 1, ACM_HALO_PHI = 2 };
+int acm_halo_plan(const acm_ctx*, int what, int side, int recv, int max_chunks, size_t* offsets, size_t* bytes);
+
+/* Launch one LB kernel on the owned planes [z0, z1) (0 <= z0 <= z1 <= owned planes; empty range = no launch)
+ * without flipping the buffers; the *_commit call flips them once all planes of the step are launched.
+ * Also valid on a plain context, where acm_step(1) equals launch(0, nz), commit for both kernels. */
+int acm_phase_launch(acm_ctx*, int z0, int z1);
+int acm_phase_commit(acm_ctx*);
+int acm_hydro_launch(acm_ctx*, int z0, int z1);
+int acm_hydro_commit(acm_ctx*);
+
 /* Parity/debug export of the populations in canonical direction order and in the storage
  * convention of the paper's two LB steps: h = post-collision values at their cell (they are
  * pulled by the next phase step), g = streamed values (collide-stream-push).

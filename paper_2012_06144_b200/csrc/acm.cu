@@ -36,8 +36,11 @@ static int fail(int code, const char* fmt, ...)
 }
 
 struct acm_ctx {
-    int nx, ny, nz, Qh, Qg, precision;
-    size_t N, esz;
+    int nx, ny, nz, Qh, Qg, precision;   // nz = allocated planes (owned planes + 2 ghost planes for a slab)
+    size_t N, esz;                        // N = nx*ny*nz: the stride between population planes
+    // slab of a z-decomposed domain (acm_create_slab); a plain context owns everything: nzl = nz, zlo = 0
+    int nzl, zlo, ghost;                  // owned planes [zlo, zlo+nzl), ghost = 1: planes zlo-1 and zlo+nzl are halos
+    int zglob0, nz_global, rank, nranks;  // global z of the first owned plane, global height, position in the decomposition
     double rho_H, rho_L, sigma, xi, M, nu_H, nu_L, grav[3];
     unsigned walls;
     cudaStream_t stream;
@@ -102,26 +105,35 @@ static int check_launch(acm_ctx* c, const char* what, cudaError_t e, int count =
 // nx is not a multiple of it (e.g. the paper's 260^3) -- a linear launch over all cells.
 static bool lb_linear(const acm_ctx* c) { return c->block.y == 1 && c->block.z == 1 && c->nx % (int)c->block.x != 0; }
 
-static Launch lb_launch(const acm_ctx* c)
+// geometry block of a launch over the owned planes [z0, z1) (relative to the first owned plane)
+static Geom geom_of(const acm_ctx* c, bool linear, int z0, int z1)
 {
-    if (lb_linear(c)) return Launch{dim3((unsigned)((c->N + c->block.x - 1) / c->block.x), 1, 1), c->block, c->stream};
-    const dim3 b = c->block;
-    return Launch{dim3((c->nx + b.x - 1) / b.x, (c->ny + b.y - 1) / b.y, (c->nz + b.z - 1) / b.z), b, c->stream};
+    Geom g;
+    g.nx = c->nx; g.ny = c->ny; g.nz = c->nz;
+    g.walls = c->walls;
+    g.linear = linear ? 1 : 0;
+    g.zlo = c->zlo; g.zhi = c->zlo + c->nzl;
+    g.zghost = c->ghost;
+    g.lz0 = c->zlo + z0; g.lz1 = c->zlo + z1;
+    return g;
+}
+static Geom geom_of(const acm_ctx* c) { return geom_of(c, false, 0, c->nzl); }
+
+static Launch launch_over(const acm_ctx* c, dim3 b, bool linear, int nplanes)
+{
+    if (linear) {
+        const size_t cells = (size_t)c->nx * c->ny * nplanes;
+        return Launch{dim3((unsigned)((cells + b.x - 1) / b.x), 1, 1), b, c->stream};
+    }
+    return Launch{dim3((c->nx + b.x - 1) / b.x, (c->ny + b.y - 1) / b.y, (nplanes + b.z - 1) / b.z), b, c->stream};
 }
 
-static dim3 grid_for(const acm_ctx* c, dim3 b)
-{
-    return dim3((c->nx + b.x - 1) / b.x, (c->ny + b.y - 1) / b.y, (c->nz + b.z - 1) / b.z);
-}
+static Launch lb_launch(const acm_ctx* c, int nplanes) { return launch_over(c, c->block, lb_linear(c), nplanes); }
 
 template <typename T> static T* wsp(acm_ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }
 
 // ---- typed implementations -----------------------------------------------------------------
-static Launch aux_launch(const acm_ctx* c)
-{
-    dim3 b(128, 1, 1);
-    return Launch{grid_for(c, b), b, c->stream};
-}
+static Launch aux_launch(const acm_ctx* c) { return launch_over(c, dim3(128, 1, 1), false, c->nzl); }
 
 template <typename T>
 static int init_t(acm_ctx* c, const void* phi, const void* u)
@@ -129,7 +141,7 @@ static int init_t(acm_ctx* c, const void* phi, const void* u)
     const bool inplace = (c->options & ACM_OPT_INPLACE) != 0;
     T *H = wsp<T>(c, c->offH[0]), *G = wsp<T>(c, c->offG[0]), *C = wsp<T>(c, c->offC[0]), *U = wsp<T>(c, c->offU[0]);
     cudaError_t e = launch_init<T>(c->Qh, c->Qg, inplace, aux_launch(c), (const T*)phi, (const T*)u, H, G, C, U,
-                                   Geom{c->nx, c->ny, c->nz, c->walls, 0}, c->N);
+                                   geom_of(c), c->N);
     if (inplace) { c->stH = ST_SWAP; c->stG = ST_IN; }
     else c->stH = c->stG = ST_POST;
     c->curH = c->curG = c->curC = c->curU = 0;
@@ -139,53 +151,77 @@ static int init_t(acm_ctx* c, const void* phi, const void* u)
 // state of the array after a step that read it in state s
 static int next_state(int s) { return s == ST_POST ? ST_POST : (s == ST_IN ? ST_SWAP : ST_IN); }
 
+// The LB kernels can be launched on a range of owned planes [z0, z1) (inner / outer split of a slab,
+// Alg. 2 lines 4-10); the buffers flip when the step is committed.
 template <typename T>
-static int launch_phase_step(acm_ctx* c)
+static int launch_phase_range(acm_ctx* c, int z0, int z1)
 {
+    if (z1 <= z0) return ACM_OK;
     PhaseArgs<T> a;
     a.Hsrc = wsp<T>(c, c->offH[c->curH]); a.Hdst = wsp<T>(c, c->offH[c->curH ^ 1]);
     a.Csrc = wsp<T>(c, c->offC[c->curC]); a.Cdst = wsp<T>(c, c->offC[c->curC ^ 1]);
     a.U = wsp<T>(c, c->offU[c->curU]);
-    a.g = Geom{c->nx, c->ny, c->nz, c->walls, lb_linear(c) ? 1 : 0};
+    a.g = geom_of(c, lb_linear(c), z0, z1);
     a.N = c->N;
     const double omega = 1.0 / (3.0 * c->M + 0.5);     // tau_phi = M/c_s^2 (eq. 2), shifted by 1/2
     a.one_minus_omega = (T)(1.0 - omega);
     a.inv_xi = (T)(1.0 / c->xi);
-    const Launch l = lb_launch(c);
+    const Launch l = lb_launch(c, z1 - z0);
     const int coll = (c->options & ACM_OPT_PHASE_SRT) ? PHASE_SRT : PHASE_MRT;
     const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
     cudaError_t e = unfused ? launch_unfused_phase<T>(c->Qh, c->walls != 0, coll, l, a)
                             : launch_phase<T>(c->Qh, c->walls != 0, c->stH, coll, l, a);
-    c->curH ^= 1; c->curC ^= 1;
-    c->stH = next_state(c->stH);
     return check_launch(c, unfused ? "stream_h/phi/collide_h kernels" : "phase_kernel", e, unfused ? 3 : 1);
 }
 
-template <typename T>
-static int launch_hydro_step(acm_ctx* c)
+static void commit_phase(acm_ctx* c)
 {
+    c->curH ^= 1; c->curC ^= 1;
+    c->stH = next_state(c->stH);
+}
+
+template <typename T>
+static int launch_hydro_range(acm_ctx* c, int z0, int z1)
+{
+    if (z1 <= z0) return ACM_OK;
     HydroArgs<T> a;
     a.Gsrc = wsp<T>(c, c->offG[c->curG]); a.Gdst = wsp<T>(c, c->offG[c->curG ^ 1]);
     a.C = wsp<T>(c, c->offC[c->curC]);
     a.U = wsp<T>(c, c->offU[c->curU]);
-    a.g = Geom{c->nx, c->ny, c->nz, c->walls, lb_linear(c) ? 1 : 0};
+    a.g = geom_of(c, lb_linear(c), z0, z1);
     a.N = c->N;
     a.rho_L = (T)c->rho_L; a.drho = (T)(c->rho_H - c->rho_L);
     a.tau_L = (T)(3.0 * c->nu_L); a.dtau = (T)(3.0 * c->nu_H - 3.0 * c->nu_L);
     a.beta4 = (T)(4.0 * 12.0 * c->sigma / c->xi); a.kappa = (T)(1.5 * c->sigma * c->xi);
     a.gx = (T)c->grav[0]; a.gy = (T)c->grav[1]; a.gz = (T)c->grav[2];
-    const Launch l = lb_launch(c);
+    const Launch l = lb_launch(c, z1 - z0);
     const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
-    cudaError_t e;
-    if (unfused) {
-        e = launch_unfused_hydro<T>(c->Qg, c->walls != 0, l, a, wsp<T>(c, c->offU[c->curU]), wsp<T>(c, c->offU[c->curU ^ 1]));
-        c->curU ^= 1;
-    } else {
-        e = launch_hydro<T>(c->Qg, c->walls != 0, c->stG, l, a);
-    }
+    cudaError_t e = unfused ? launch_unfused_hydro<T>(c->Qg, c->walls != 0, l, a, wsp<T>(c, c->offU[c->curU]), wsp<T>(c, c->offU[c->curU ^ 1]))
+                            : launch_hydro<T>(c->Qg, c->walls != 0, c->stG, l, a);
+    return check_launch(c, unfused ? "stream_g/velocity/collide_g kernels" : "hydro_kernel", e, unfused ? 3 : 1);
+}
+
+static void commit_hydro(acm_ctx* c)
+{
+    if (c->options & ACM_OPT_UNFUSED) c->curU ^= 1;
     c->curG ^= 1;
     c->stG = next_state(c->stG);
-    return check_launch(c, unfused ? "stream_g/velocity/collide_g kernels" : "hydro_kernel", e, unfused ? 3 : 1);
+}
+
+template <typename T>
+static int launch_phase_step(acm_ctx* c)
+{
+    int rc = launch_phase_range<T>(c, 0, c->nzl);
+    if (rc == ACM_OK) commit_phase(c);
+    return rc;
+}
+
+template <typename T>
+static int launch_hydro_step(acm_ctx* c)
+{
+    int rc = launch_hydro_range<T>(c, 0, c->nzl);
+    if (rc == ACM_OK) commit_hydro(c);
+    return rc;
 }
 
 static void prof_mark(acm_ctx* c)
@@ -216,7 +252,7 @@ template <typename T>
 static int export_g_t(acm_ctx* c, void* g, void* p)      // incoming convention (+ pressure)
 {
     cudaError_t e = launch_export<T>(c->Qg, c->stG, false, aux_launch(c), wsp<T>(c, c->offG[c->curG]), wsp<T>(c, c->offC[c->curC]),
-                                     (T*)g, (T*)p, Geom{c->nx, c->ny, c->nz, c->walls, 0}, c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L));
+                                     (T*)g, (T*)p, geom_of(c), c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L));
     return check_launch(c, "export_kernel", e);
 }
 
@@ -224,7 +260,7 @@ template <typename T>
 static int export_h_t(acm_ctx* c, void* h)               // post-collision convention
 {
     cudaError_t e = launch_export<T>(c->Qh, c->stH, true, aux_launch(c), wsp<T>(c, c->offH[c->curH]), wsp<T>(c, c->offC[c->curC]),
-                                     (T*)h, (T*)nullptr, Geom{c->nx, c->ny, c->nz, c->walls, 0}, c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L));
+                                     (T*)h, (T*)nullptr, geom_of(c), c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L));
     return check_launch(c, "export_kernel", e);
 }
 
@@ -232,7 +268,7 @@ template <typename T>
 static int import_g_t(acm_ctx* c, const void* g)      // incoming convention -> ST_POST storage
 {
     cudaError_t e = launch_import<T>(c->Qg, false, aux_launch(c), (const T*)g, wsp<T>(c, c->offG[c->curG]),
-                                     Geom{c->nx, c->ny, c->nz, c->walls, 0}, c->N);
+                                     geom_of(c), c->N);
     return check_launch(c, "import_kernel", e);
 }
 
@@ -240,7 +276,7 @@ template <typename T>
 static int import_h_t(acm_ctx* c, const void* h)      // post-collision convention -> ST_SWAP storage
 {
     cudaError_t e = launch_import<T>(c->Qh, true, aux_launch(c), (const T*)h, wsp<T>(c, c->offH[c->curH]),
-                                     Geom{c->nx, c->ny, c->nz, c->walls, 0}, c->N);
+                                     geom_of(c), c->N);
     return check_launch(c, "import_kernel", e);
 }
 
@@ -257,6 +293,64 @@ static int copy_async(acm_ctx* c, void* dst, const void* src, size_t bytes, cuda
 #define ACM_CHECK_CTX(c)                                                          \
     if (!(c)) return fail(ACM_EINVAL, "%s: NULL context", __func__);              \
     if ((c)->sticky) return fail(ACM_ECUDA, "%s: context has a sticky CUDA error", __func__)
+
+// nz = owned planes; rank/nranks/nz_global/zglob0 describe the slab (nranks = 0: a plain context without ghost planes)
+static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int stencil_hydro, double rho_H, double rho_L,
+                       double sigma, double xi, double M, double nu_H, double nu_L, const double gravity[3], unsigned wall_flags,
+                       int precision, unsigned options, void* workspace, void* cuda_stream, int rank, int nranks, int nz_global,
+                       int zglob0)
+{
+    const bool slab = nranks > 0;
+    const int nzl = nz;
+    if (slab) {
+        if (options & (ACM_OPT_INPLACE | ACM_OPT_UNFUSED))
+            return fail(ACM_EINVAL, "acm_create_slab: ACM_OPT_INPLACE / ACM_OPT_UNFUSED are not available for slabs");
+        if (nz > 0) nz += 2;      // ghost planes below and above
+    }
+    if (!out) return fail(ACM_EINVAL, "acm_create: out is NULL");
+    *out = nullptr;
+    Layout L;
+    if (!make_layout(nx, ny, nz, stencil_phase, stencil_hydro, precision, options, &L))
+        return fail(ACM_EINVAL, "acm_create: invalid size (%d,%d,%d), stencils (%d,%d), precision %d or options %u", nx, ny, nz,
+                    stencil_phase, stencil_hydro, precision, options);
+    if (!(rho_L > 0.0) || !(rho_H >= rho_L)) return fail(ACM_EINVAL, "acm_create: need rho_H >= rho_L > 0");
+    if (!(xi > 0.0)) return fail(ACM_EINVAL, "acm_create: need xi > 0");
+    if (!(sigma >= 0.0)) return fail(ACM_EINVAL, "acm_create: need sigma >= 0");
+    if (!(M > 0.0) || !std::isfinite(M)) return fail(ACM_EINVAL, "acm_create: need mobility M > 0");
+    if (!(nu_H > 0.0) || !(nu_L > 0.0)) return fail(ACM_EINVAL, "acm_create: need nu_H, nu_L > 0");
+    if (wall_flags & ~7u) return fail(ACM_EINVAL, "acm_create: unknown wall flag");
+    if (!workspace) return fail(ACM_EINVAL, "acm_create: workspace is NULL");
+    if ((uintptr_t)workspace & 255) return fail(ACM_EINVAL, "acm_create: workspace must be 256-byte aligned");
+    acm_ctx* c = new (std::nothrow) acm_ctx();
+    if (!c) return fail(ACM_EINVAL, "acm_create: out of host memory");
+    c->nx = nx; c->ny = ny; c->nz = nz; c->Qh = stencil_phase; c->Qg = stencil_hydro; c->precision = precision;
+    c->N = (size_t)nx * ny * nz; c->esz = precision == ACM_F64 ? 8 : 4;
+    c->rho_H = rho_H; c->rho_L = rho_L; c->sigma = sigma; c->xi = xi; c->M = M; c->nu_H = nu_H; c->nu_L = nu_L;
+    for (int a = 0; a < 3; ++a) c->grav[a] = gravity ? gravity[a] : 0.0;
+    // internal wall bits: the z walls per face; a slab has a z wall only on an outer face of the domain
+    c->walls = wall_flags & (ACM_WALL_X | ACM_WALL_Y);
+    if (wall_flags & ACM_WALL_Z) {
+        if (!slab || rank == 0) c->walls |= WALL_ZLO;
+        if (!slab || rank == nranks - 1) c->walls |= WALL_ZHI;
+    }
+    c->nzl = nzl; c->zlo = slab ? 1 : 0; c->ghost = slab ? 1 : 0;
+    c->zglob0 = zglob0; c->nz_global = slab ? nz_global : nzl; c->rank = slab ? rank : 0; c->nranks = slab ? nranks : 1;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->ws = (char*)workspace;
+    for (int b = 0; b < 2; ++b) { c->offH[b] = L.offH[b]; c->offG[b] = L.offG[b]; c->offC[b] = L.offC[b]; }
+    c->offU[0] = L.offU[0]; c->offU[1] = L.offU[1]; c->offStage = L.offStage; c->offRed = L.offRed;
+    c->curH = c->curG = c->curC = c->curU = 0;
+    c->options = options;
+    c->stH = c->stG = ST_POST;
+    c->initialised = false;
+    c->sticky = ACM_OK;
+    c->block = dim3(128, 1, 1);
+    c->launches = 0;
+    c->profiling = false;
+    *out = c;
+    return ACM_OK;
+}
+
 
 // ---- C ABI ----------------------------------------------------------------------------------
 extern "C" {
@@ -286,40 +380,120 @@ int acm_create_opt(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int
                    double sigma, double xi, double M, double nu_H, double nu_L, const double gravity[3], unsigned wall_flags,
                    int precision, unsigned options, void* workspace, void* cuda_stream)
 {
-    if (!out) return fail(ACM_EINVAL, "acm_create: out is NULL");
-    *out = nullptr;
-    Layout L;
-    if (!make_layout(nx, ny, nz, stencil_phase, stencil_hydro, precision, options, &L))
-        return fail(ACM_EINVAL, "acm_create: invalid size (%d,%d,%d), stencils (%d,%d), precision %d or options %u", nx, ny, nz,
-                    stencil_phase, stencil_hydro, precision, options);
-    if (!(rho_L > 0.0) || !(rho_H >= rho_L)) return fail(ACM_EINVAL, "acm_create: need rho_H >= rho_L > 0");
-    if (!(xi > 0.0)) return fail(ACM_EINVAL, "acm_create: need xi > 0");
-    if (!(sigma >= 0.0)) return fail(ACM_EINVAL, "acm_create: need sigma >= 0");
-    if (!(M > 0.0) || !std::isfinite(M)) return fail(ACM_EINVAL, "acm_create: need mobility M > 0");
-    if (!(nu_H > 0.0) || !(nu_L > 0.0)) return fail(ACM_EINVAL, "acm_create: need nu_H, nu_L > 0");
-    if (wall_flags & ~7u) return fail(ACM_EINVAL, "acm_create: unknown wall flag");
-    if (!workspace) return fail(ACM_EINVAL, "acm_create: workspace is NULL");
-    if ((uintptr_t)workspace & 255) return fail(ACM_EINVAL, "acm_create: workspace must be 256-byte aligned");
-    acm_ctx* c = new (std::nothrow) acm_ctx();
-    if (!c) return fail(ACM_EINVAL, "acm_create: out of host memory");
-    c->nx = nx; c->ny = ny; c->nz = nz; c->Qh = stencil_phase; c->Qg = stencil_hydro; c->precision = precision;
-    c->N = (size_t)nx * ny * nz; c->esz = precision == ACM_F64 ? 8 : 4;
-    c->rho_H = rho_H; c->rho_L = rho_L; c->sigma = sigma; c->xi = xi; c->M = M; c->nu_H = nu_H; c->nu_L = nu_L;
-    for (int a = 0; a < 3; ++a) c->grav[a] = gravity ? gravity[a] : 0.0;
-    c->walls = wall_flags;
-    c->stream = (cudaStream_t)cuda_stream;
-    c->ws = (char*)workspace;
-    for (int b = 0; b < 2; ++b) { c->offH[b] = L.offH[b]; c->offG[b] = L.offG[b]; c->offC[b] = L.offC[b]; }
-    c->offU[0] = L.offU[0]; c->offU[1] = L.offU[1]; c->offStage = L.offStage; c->offRed = L.offRed;
-    c->curH = c->curG = c->curC = c->curU = 0;
-    c->options = options;
-    c->stH = c->stG = ST_POST;
-    c->initialised = false;
-    c->sticky = ACM_OK;
-    c->block = dim3(128, 1, 1);
-    c->launches = 0;
-    c->profiling = false;
-    *out = c;
+    return create_impl(out, nx, ny, nz, stencil_phase, stencil_hydro, rho_H, rho_L, sigma, xi, M, nu_H, nu_L, gravity, wall_flags,
+                       precision, options, workspace, cuda_stream, 0, 0, nz, 0);
+}
+
+// ---- slab decomposition along z --------------------------------------------------------------
+int acm_slab_range(int nz_global, int rank, int nranks, int* z_begin, int* z_count)
+{
+    if (nz_global < 1 || nranks < 1 || rank < 0 || rank >= nranks || nranks > nz_global)
+        return fail(ACM_EINVAL, "acm_slab_range: need 1 <= nranks <= nz_global and 0 <= rank < nranks");
+    const int base = nz_global / nranks, rem = nz_global % nranks;     // the first `rem` slabs get one more plane
+    if (z_begin) *z_begin = rank * base + (rank < rem ? rank : rem);
+    if (z_count) *z_count = base + (rank < rem ? 1 : 0);
+    return ACM_OK;
+}
+
+size_t acm_workspace_bytes_slab(int nx, int ny, int nz_global, int stencil_phase, int stencil_hydro, int precision, int rank,
+                                int nranks)
+{
+    int z0, cnt;
+    if (acm_slab_range(nz_global, rank, nranks, &z0, &cnt) != ACM_OK) return 0;
+    return acm_workspace_bytes_opt(nx, ny, cnt + 2, stencil_phase, stencil_hydro, precision, 0u);
+}
+
+int acm_create_slab(acm_ctx** out, int nx, int ny, int nz_global, int stencil_phase, int stencil_hydro, double rho_H,
+                    double rho_L, double sigma, double xi, double M, double nu_H, double nu_L, const double gravity[3],
+                    unsigned wall_flags, int precision, unsigned options, int rank, int nranks, void* workspace,
+                    void* cuda_stream)
+{
+    if (out) *out = nullptr;
+    int z0, cnt;
+    int rc = acm_slab_range(nz_global, rank, nranks, &z0, &cnt);
+    if (rc) return rc;
+    return create_impl(out, nx, ny, cnt, stencil_phase, stencil_hydro, rho_H, rho_L, sigma, xi, M, nu_H, nu_L, gravity, wall_flags,
+                       precision, options, workspace, cuda_stream, rank, nranks, nz_global, z0);
+}
+
+int acm_slab_info(const acm_ctx* c, int info[6])
+{
+    if (!c || !info) return fail(ACM_EINVAL, "acm_slab_info: NULL argument");
+    info[0] = c->rank; info[1] = c->nranks; info[2] = c->zglob0; info[3] = c->nzl; info[4] = c->nz; info[5] = c->ghost;
+    return ACM_OK;
+}
+
+// planes that cross a z face: directions with e_z = +1 (sign > 0) or e_z = -1 (sign < 0), increasing index
+static int crossing_dirs(int Q, int sign, int* dirs)
+{
+    int n = 0;
+    for (int i = 0; i < Q; ++i) {
+        const int k = (Q == 15 && i >= 7) ? i + 12 : i;
+        if (acm::dir27(k, 2) == sign) dirs[n++] = i;
+    }
+    return n;
+}
+
+int acm_halo_plan(const acm_ctx* c, int what, int side, int recv, int max_chunks, size_t* offsets, size_t* bytes)
+{
+    if (!c || !offsets || !bytes) return -fail(ACM_EINVAL, "acm_halo_plan: NULL argument");
+    if (!c->ghost) return -fail(ACM_ESTATE, "acm_halo_plan: not a slab context");
+    if ((what != ACM_HALO_H && what != ACM_HALO_G && what != ACM_HALO_PHI) || (side != 0 && side != 1))
+        return -fail(ACM_EINVAL, "acm_halo_plan: bad what/side");
+    const size_t plane = (size_t)c->nx * c->ny * c->esz;
+    // side 0 = low z face: my first owned plane (zlo) goes out, my low ghost plane (zlo-1) comes in;
+    // side 1 = high z face: my last owned plane goes out, my high ghost plane comes in
+    const int zplane = side == 0 ? (recv ? c->zlo - 1 : c->zlo) : (recv ? c->zlo + c->nzl : c->zlo + c->nzl - 1);
+    int n = 0;
+    if (what == ACM_HALO_PHI) {
+        if (max_chunks < 1) return -fail(ACM_EINVAL, "acm_halo_plan: max_chunks too small");
+        offsets[0] = c->offC[c->curC] + (size_t)zplane * plane;
+        bytes[0] = plane;
+        return 1;
+    }
+    // Populations are stored post-collision at their own cell and pulled by the next step: the cell at z
+    // pulls slot i from z - e_iz.  My low ghost plane must hold the slots with e_z = +1 (pulled upwards into my
+    // first plane); what I send through the low face fills the low neighbour's HIGH ghost: slots with e_z = -1.
+    const int Q = what == ACM_HALO_H ? c->Qh : c->Qg;
+    const size_t base = what == ACM_HALO_H ? c->offH[c->curH] : c->offG[c->curG];
+    const int sign = (side == 0) == (recv != 0) ? +1 : -1;
+    int dirs[27];
+    n = crossing_dirs(Q, sign, dirs);
+    if (n > max_chunks) return -fail(ACM_EINVAL, "acm_halo_plan: max_chunks too small (need %d)", n);
+    for (int k = 0; k < n; ++k) {
+        offsets[k] = base + ((size_t)dirs[k] * c->N) * c->esz + (size_t)zplane * plane;
+        bytes[k] = plane;
+    }
+    return n;
+}
+
+int acm_phase_launch(acm_ctx* c, int z0, int z1)
+{
+    ACM_CHECK_CTX(c);
+    if (!c->initialised) return fail(ACM_ESTATE, "acm_phase_launch: call acm_init first");
+    if (z0 < 0 || z1 > c->nzl || z0 > z1) return fail(ACM_EINVAL, "acm_phase_launch: need 0 <= z0 <= z1 <= owned planes");
+    return c->precision == ACM_F64 ? launch_phase_range<double>(c, z0, z1) : launch_phase_range<float>(c, z0, z1);
+}
+
+int acm_phase_commit(acm_ctx* c)
+{
+    ACM_CHECK_CTX(c);
+    commit_phase(c);
+    return ACM_OK;
+}
+
+int acm_hydro_launch(acm_ctx* c, int z0, int z1)
+{
+    ACM_CHECK_CTX(c);
+    if (!c->initialised) return fail(ACM_ESTATE, "acm_hydro_launch: call acm_init first");
+    if (z0 < 0 || z1 > c->nzl || z0 > z1) return fail(ACM_EINVAL, "acm_hydro_launch: need 0 <= z0 <= z1 <= owned planes");
+    return c->precision == ACM_F64 ? launch_hydro_range<double>(c, z0, z1) : launch_hydro_range<float>(c, z0, z1);
+}
+
+int acm_hydro_commit(acm_ctx* c)
+{
+    ACM_CHECK_CTX(c);
+    commit_hydro(c);
     return ACM_OK;
 }
 
@@ -387,6 +561,14 @@ int acm_init(acm_ctx* c, const void* phi, const void* u)
     ACM_CHECK_CTX(c);
     if (!phi || !u) return fail(ACM_EINVAL, "acm_init: phi and u are required");
     int rc = c->precision == ACM_F64 ? init_t<double>(c, phi, u) : init_t<float>(c, phi, u);
+    if (rc == ACM_OK && c->ghost) {
+        // slab: phi and u come with their ghost planes filled (the pre-shifted g needs u of the neighbour planes);
+        // the phi ghost planes are taken over as they are, those of h and g arrive with the first halo exchange
+        const size_t plane = (size_t)c->nx * c->ny * c->esz;
+        const size_t hi = (size_t)(c->zlo + c->nzl) * plane;
+        rc = copy_async(c, c->ws + c->offC[0], phi, plane, cudaMemcpyDeviceToDevice, "acm_init(phi ghost)");
+        if (!rc) rc = copy_async(c, c->ws + c->offC[0] + hi, (const char*)phi + hi, plane, cudaMemcpyDeviceToDevice, "acm_init(phi ghost)");
+    }
     if (rc == ACM_OK) c->initialised = true;
     return rc;
 }
@@ -396,6 +578,7 @@ int acm_step(acm_ctx* c, int n)
     ACM_CHECK_CTX(c);
     if (n < 0) return fail(ACM_EINVAL, "acm_step: n must be >= 0");
     if (!c->initialised) return fail(ACM_ESTATE, "acm_step: call acm_init first");
+    if (c->ghost && n > 0) return fail(ACM_ESTATE, "acm_step: a slab advances with acm_phase_launch / acm_hydro_launch and the halo exchange");
     return c->precision == ACM_F64 ? step_t<double>(c, n) : step_t<float>(c, n);
 }
 
@@ -416,8 +599,9 @@ int acm_phi_mass(acm_ctx* c, double* total_host)
     if (!total_host) return fail(ACM_EINVAL, "acm_phi_mass: total_host is NULL");
     if (!c->initialised) return fail(ACM_ESTATE, "acm_phi_mass: call acm_init first");
     double* part = wsp<double>(c, c->offRed);
-    cudaError_t le = c->precision == ACM_F64 ? launch_sum_phi<double>(c->stream, wsp<double>(c, c->offC[c->curC]), c->N, part)
-                                             : launch_sum_phi<float>(c->stream, wsp<float>(c, c->offC[c->curC]), c->N, part);
+    const size_t first = (size_t)c->zlo * c->nx * c->ny, owned = (size_t)c->nzl * c->nx * c->ny;   // a slab sums its own planes
+    cudaError_t le = c->precision == ACM_F64 ? launch_sum_phi<double>(c->stream, wsp<double>(c, c->offC[c->curC]) + first, owned, part)
+                                             : launch_sum_phi<float>(c->stream, wsp<float>(c, c->offC[c->curC]) + first, owned, part);
     int rc = check_launch(c, "sum_phi", le, 2);
     if (rc) return rc;
     rc = copy_async(c, total_host, part + RED_BLOCKS, sizeof(double), cudaMemcpyDeviceToHost, "acm_phi_mass");
@@ -428,23 +612,32 @@ int acm_phi_mass(acm_ctx* c, double* total_host)
     return ACM_OK;
 }
 
-int acm_bubble_diag(acm_ctx* c, double out_host[7])
+int acm_bubble_sums(acm_ctx* c, double out_host[7])
 {
     ACM_CHECK_CTX(c);
-    if (!out_host) return fail(ACM_EINVAL, "acm_bubble_diag: out_host is NULL");
-    if (!c->initialised) return fail(ACM_ESTATE, "acm_bubble_diag: call acm_init first");
+    if (!out_host) return fail(ACM_EINVAL, "acm_bubble_sums: out_host is NULL");
+    if (!c->initialised) return fail(ACM_ESTATE, "acm_bubble_sums: call acm_init first");
     double* part = wsp<double>(c, c->offRed);
-    const Geom g{c->nx, c->ny, c->nz, c->walls};
+    const Geom g = geom_of(c);
+    const int zshift = c->zglob0 - c->zlo;
     cudaError_t le = c->precision == ACM_F64
-                         ? launch_bubble_diag<double>(c->stream, wsp<double>(c, c->offC[c->curC]), wsp<double>(c, c->offU[c->curU]), g, c->N, part)
-                         : launch_bubble_diag<float>(c->stream, wsp<float>(c, c->offC[c->curC]), wsp<float>(c, c->offU[c->curU]), g, c->N, part);
+                         ? launch_bubble_diag<double>(c->stream, wsp<double>(c, c->offC[c->curC]), wsp<double>(c, c->offU[c->curU]), g, c->N, zshift, part)
+                         : launch_bubble_diag<float>(c->stream, wsp<float>(c, c->offC[c->curC]), wsp<float>(c, c->offU[c->curU]), g, c->N, zshift, part);
     int rc = check_launch(c, "bubble_diag", le, 2);
     if (rc) return rc;
-    double sums[DIAG_WIDTH];
-    rc = copy_async(c, sums, part + (size_t)DIAG_WIDTH * RED_BLOCKS, sizeof(sums), cudaMemcpyDeviceToHost, "acm_bubble_diag");
+    rc = copy_async(c, out_host, part + (size_t)DIAG_WIDTH * RED_BLOCKS, DIAG_WIDTH * sizeof(double), cudaMemcpyDeviceToHost, "acm_bubble_sums");
     if (rc) return rc;
     cudaError_t e = cudaStreamSynchronize(c->stream);
-    if (e != cudaSuccess) { c->sticky = ACM_ECUDA; return fail(ACM_ECUDA, "acm_bubble_diag: %s", cudaGetErrorString(e)); }
+    if (e != cudaSuccess) { c->sticky = ACM_ECUDA; return fail(ACM_ECUDA, "acm_bubble_sums: %s", cudaGetErrorString(e)); }
+    return ACM_OK;
+}
+
+int acm_bubble_diag(acm_ctx* c, double out_host[7])
+{
+    if (!out_host) return fail(ACM_EINVAL, "acm_bubble_diag: out_host is NULL");
+    double sums[DIAG_WIDTH];
+    int rc = acm_bubble_sums(c, sums);
+    if (rc) return rc;
     out_host[0] = sums[0];
     for (int k = 1; k < DIAG_WIDTH; ++k) out_host[k] = sums[k] / sums[0];
     for (int k = 0; k < DIAG_WIDTH; ++k)
@@ -515,6 +708,7 @@ int acm_run_host(acm_ctx* c, const void* phi_host, const void* u_host, int n, vo
     ACM_CHECK_CTX(c);
     if (!phi_host || !u_host) return fail(ACM_EINVAL, "acm_run_host: phi_host and u_host are required");
     if (n < 0) return fail(ACM_EINVAL, "acm_run_host: n must be >= 0");
+    if (c->ghost) return fail(ACM_ESTATE, "acm_run_host: not available for a slab (its steps need the halo exchange)");
     const size_t fb = c->N * c->esz;
     char* st = c->ws + c->offStage;
     int rc = copy_async(c, st, phi_host, fb, cudaMemcpyHostToDevice, "acm_run_host(h2d phi)");

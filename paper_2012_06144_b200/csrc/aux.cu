@@ -22,10 +22,8 @@ __device__ __forceinline__ T gamma_i(int ex, int ey, int ez, T w, T ux, T uy, T 
 template <typename T, int QH, int QG, bool INPLACE>
 __global__ void init_kernel(const T* __restrict__ phi, const T* __restrict__ u, T* H, T* G, T* C, T* U, Geom g, size_t N)
 {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x;
-    const int y = blockIdx.y * blockDim.y + threadIdx.y;
-    const int z = blockIdx.z * blockDim.z + threadIdx.z;
-    if (x >= g.nx || y >= g.ny || z >= g.nz) return;
+    int x, y, z;
+    if (!cell_of_thread(g, x, y, z)) return;
     Nbr nb;
     nb.setup<true>(g, x, y, z);
     const int idx = nb.at<0, 0, 0>();
@@ -65,10 +63,8 @@ __global__ void init_kernel(const T* __restrict__ phi, const T* __restrict__ u, 
 template <typename T, int Q, int STATE, bool POST>
 __global__ void export_kernel(const T* F, const T* __restrict__ C, T* out, T* p, Geom g, size_t N, T rho_L, T drho)
 {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x;
-    const int y = blockIdx.y * blockDim.y + threadIdx.y;
-    const int z = blockIdx.z * blockDim.z + threadIdx.z;
-    if (x >= g.nx || y >= g.ny || z >= g.nz) return;
+    int x, y, z;
+    if (!cell_of_thread(g, x, y, z)) return;
     Nbr nb;
     nb.setup<true>(g, x, y, z);
     const int idx = nb.at<0, 0, 0>();
@@ -89,10 +85,8 @@ __global__ void export_kernel(const T* F, const T* __restrict__ C, T* out, T* p,
 template <typename T, int Q, bool POST>
 __global__ void import_kernel(const T* __restrict__ in, T* F, Geom g, size_t N)
 {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x;
-    const int y = blockIdx.y * blockDim.y + threadIdx.y;
-    const int z = blockIdx.z * blockDim.z + threadIdx.z;
-    if (x >= g.nx || y >= g.ny || z >= g.nz) return;
+    int x, y, z;
+    if (!cell_of_thread(g, x, y, z)) return;
     Nbr nb;
     nb.setup<true>(g, x, y, z);
     const int idx = nb.at<0, 0, 0>();
@@ -149,13 +143,16 @@ __global__ void __launch_bounds__(RED_THREADS) sum_pass2(const double* __restric
 // light-phase indicator 1 - phi:  V, V x_c, V y_c, V z_c (cell centres i + 1/2), V u_x, V u_y, V u_z.
 // Same fixed-order two-pass scheme as sum(phi), so the result is bitwise reproducible.
 template <typename T>
-__global__ void __launch_bounds__(RED_THREADS) diag_pass1(const T* __restrict__ C, const T* __restrict__ U, Geom g, size_t N, double* part)
+__global__ void __launch_bounds__(RED_THREADS) diag_pass1(const T* __restrict__ C, const T* __restrict__ U, Geom g, size_t N, int zshift, double* part)
 {
+    // cells of the owned planes [zlo, zhi); z coordinate reported in the global frame (slab: + zshift)
     double s[DIAG_WIDTH] = {0, 0, 0, 0, 0, 0, 0};
     const size_t plane = (size_t)g.nx * g.ny;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
-        const int z = (int)(i / plane);
-        const int r = (int)(i - (size_t)z * plane);
+    const size_t end = (size_t)g.zhi * plane;
+    for (size_t i = (size_t)g.zlo * plane + (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < end; i += (size_t)gridDim.x * blockDim.x) {
+        const int zl = (int)(i / plane);
+        const int r = (int)(i - (size_t)zl * plane);
+        const int z = zl + zshift;
         const int y = r / g.nx, x = r - y * g.nx;
         const double w = 1.0 - (double)C[i];
         s[0] += w;
@@ -238,9 +235,9 @@ cudaError_t launch_sum_phi(cudaStream_t s, const T* C, size_t N, double* part)
 }
 
 template <typename T>
-cudaError_t launch_bubble_diag(cudaStream_t s, const T* C, const T* U, Geom g, size_t N, double* part)
+cudaError_t launch_bubble_diag(cudaStream_t s, const T* C, const T* U, Geom g, size_t N, int zshift, double* part)
 {
-    diag_pass1<T><<<RED_BLOCKS, RED_THREADS, 0, s>>>(C, U, g, N, part);
+    diag_pass1<T><<<RED_BLOCKS, RED_THREADS, 0, s>>>(C, U, g, N, zshift, part);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     diag_pass2<<<DIAG_WIDTH, RED_THREADS, 0, s>>>(part, part + (size_t)DIAG_WIDTH * RED_BLOCKS);
@@ -252,7 +249,7 @@ cudaError_t launch_bubble_diag(cudaStream_t s, const T* C, const T* U, Geom g, s
     template cudaError_t launch_export<T>(int, int, bool, const Launch&, const T*, const T*, T*, T*, Geom, size_t, T, T);   \
     template cudaError_t launch_import<T>(int, bool, const Launch&, const T*, T*, Geom, size_t);                            \
     template cudaError_t launch_sum_phi<T>(cudaStream_t, const T*, size_t, double*);                                        \
-    template cudaError_t launch_bubble_diag<T>(cudaStream_t, const T*, const T*, Geom, size_t, double*);
+    template cudaError_t launch_bubble_diag<T>(cudaStream_t, const T*, const T*, Geom, size_t, int, double*);
 ACM_INSTANTIATE_AUX(double)
 ACM_INSTANTIATE_AUX(float)
 

@@ -15,28 +15,37 @@ namespace acm {
 // ------------------------------------------------------------------------------------------
 // geometry: neighbour indexing with periodic wrap, wall flags for half-way bounce-back
 // ------------------------------------------------------------------------------------------
+// Internal wall bits: ACM_WALL_X, ACM_WALL_Y as in the ABI; the z walls are kept per face because a
+// slab of a z-decomposed domain (acm_create_slab) has a wall on at most one of its faces.
+enum { WALL_ZLO = 4, WALL_ZHI = 8 };
+
 struct Geom {
-    int nx, ny, nz;
-    unsigned walls;
+    int nx, ny, nz;  // allocated planes: nz includes the two ghost planes of a slab
+    unsigned walls;  // ACM_WALL_X | ACM_WALL_Y | WALL_ZLO | WALL_ZHI
     int linear;      // 1: the launch is 1-D over all cells (rows not a multiple of the block: no idle tail threads)
+    int zlo, zhi;    // planes [zlo, zhi) are the cells this context owns ([0, nz) without ghost planes)
+    int zghost;      // 1: planes zlo-1 and zhi hold the neighbour slabs' boundary planes (no periodic wrap in z)
+    int lz0, lz1;    // planes [lz0, lz1) are covered by this launch (inner / outer split of a slab)
 };
 
-// cell of the calling thread: 3-D launch (block tiles of x-rows) or linear launch over the N cells
+// cell of the calling thread: 3-D launch (block tiles of x-rows) or linear launch over the cells of
+// the planes [lz0, lz1)
 __device__ __forceinline__ bool cell_of_thread(const Geom& g, int& x, int& y, int& z)
 {
     if (g.linear) {
         const unsigned id = blockIdx.x * blockDim.x + threadIdx.x;
-        if (id >= (unsigned)(g.nx * g.ny * g.nz)) return false;
+        if (id >= (unsigned)(g.nx * g.ny * (g.lz1 - g.lz0))) return false;
         const unsigned t = id / (unsigned)g.nx;
         x = (int)(id - t * (unsigned)g.nx);
-        z = (int)(t / (unsigned)g.ny);
-        y = (int)(t - (unsigned)z * (unsigned)g.ny);
+        const unsigned zr = t / (unsigned)g.ny;
+        y = (int)(t - zr * (unsigned)g.ny);
+        z = g.lz0 + (int)zr;
         return true;
     }
     x = blockIdx.x * blockDim.x + threadIdx.x;
     y = blockIdx.y * blockDim.y + threadIdx.y;
-    z = blockIdx.z * blockDim.z + threadIdx.z;
-    return x < g.nx && y < g.ny && z < g.nz;
+    z = g.lz0 + blockIdx.z * blockDim.z + threadIdx.z;
+    return x < g.nx && y < g.ny && z < g.lz1;
 }
 
 // Per-cell neighbourhood: coordinates of x-1, x, x+1 (periodic wrap; clamped at a wall, which is
@@ -55,8 +64,9 @@ struct Nbr {
         if (xp >= g.nx) { if (WALLS && (g.walls & ACM_WALL_X)) { wxp = true; xp = g.nx - 1; } else xp = 0; }
         if (ym < 0) { if (WALLS && (g.walls & ACM_WALL_Y)) { wym = true; ym = 0; } else ym = g.ny - 1; }
         if (yp >= g.ny) { if (WALLS && (g.walls & ACM_WALL_Y)) { wyp = true; yp = g.ny - 1; } else yp = 0; }
-        if (zm < 0) { if (WALLS && (g.walls & ACM_WALL_Z)) { wzm = true; zm = 0; } else zm = g.nz - 1; }
-        if (zp >= g.nz) { if (WALLS && (g.walls & ACM_WALL_Z)) { wzp = true; zp = g.nz - 1; } else zp = 0; }
+        // z: wall -> clamp; ghost planes -> use them as they are; else periodic wrap inside [zlo, zhi)
+        if (zm < g.zlo) { if (WALLS && (g.walls & WALL_ZLO)) { wzm = true; zm = g.zlo; } else if (!g.zghost) zm = g.zhi - 1; }
+        if (zp >= g.zhi) { if (WALLS && (g.walls & WALL_ZHI)) { wzp = true; zp = g.zhi - 1; } else if (!g.zghost) zp = g.zlo; }
         xs[0] = xm; xs[1] = x; xs[2] = xp;
         const int ys[3] = {ym, y, yp}, zs[3] = {zm, z, zp};
 #pragma unroll

@@ -38,6 +38,7 @@ template <typename T> cudaError_t launch_import(int Q, bool post, const Launch& 
 constexpr int RED_BLOCKS = 592, RED_THREADS = 256;   // 4 CTAs per SM on 148 SMs
 constexpr int DIAG_WIDTH = 7;                        // V, V*x, V*y, V*z, V*ux, V*uy, V*uz
 template <typename T> cudaError_t launch_sum_phi(cudaStream_t s, const T* C, size_t N, double* part);
-template <typename T> cudaError_t launch_bubble_diag(cudaStream_t s, const T* C, const T* U, Geom g, size_t N, double* part);
+// launch_bubble_diag sums over the owned planes [g.zlo, g.zhi); zshift = global z of plane 0 (slabs).
+template <typename T> cudaError_t launch_bubble_diag(cudaStream_t s, const T* C, const T* U, Geom g, size_t N, int zshift, double* part);
 
 }  // namespace acm
