@@ -286,6 +286,90 @@ def run_acm(args, rank, local_rank, world):
     replicas.shutdown()
 
 
+def run_decomposed(args, rank, local_rank, world):
+    """--decompose: ONE global domain cut into z-slabs, one per rank (outside north_star, which
+    is a single GPU).  Weak scaling: every rank owns a full copy of the workload's grid, the global domain is
+    their stack along z (the workloads are periodic in z, so the stacked field is continuous); the ranks
+    exchange halo planes every step (slab.py).  Not the default: `--gpus N` alone runs replicas."""
+    import torch
+    from paper_2012_06144_b200 import replicas
+    from paper_2012_06144_b200.slab import SlabRunner, pad_planes
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    replicas.init("nccl", dev)
+    K, W = args.steps, max(args.warmup, 3)
+    p, phi, u, name = workload(args.config)
+    if p.wall_flags & 4:
+        raise SystemExit("--decompose stacks the workload along z: it must be periodic in z")
+    precision = args.precision
+    esz = 8 if precision == "f64" else 4
+    np_dtype = "float64" if precision == "f64" else "float32"
+    phi_h = torch.from_numpy(phi.astype(np_dtype)).pin_memory()
+    u_h = torch.from_numpy(u.astype(np_dtype)).pin_memory()
+    pg = p.replace(nz=p.nz * world)
+    run = SlabRunner.distributed(pg, rank, world, precision=precision, device=dev, overlap=not args.no_overlap)
+    slab = run.slabs[0]
+
+    def load():
+        slab.init(pad_planes(phi_h.to(dev, non_blocking=True), 0, p.nz), pad_planes(u_h.to(dev, non_blocking=True), 0, p.nz))
+        run.refresh_halos()
+
+    load()
+    run.step(W)
+    replicas.barrier(dev)
+    launches0 = slab.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clk:
+        e0.record()
+        run.step(K)
+        run.sync_halos()
+        e1.record()
+        replicas.barrier(dev)
+    ms = replicas.max_over_ranks(e0.elapsed_time(e1), dev)
+    launches = slab.launch_count - launches0
+    N = p.ncells
+    value = replicas.aggregate_mlups(N, K, ms, world)
+    mass = slab.phi_mass()
+    # end to end: host -> device, init, halos, K steps, fields -> host
+    po, uo = torch.empty_like(phi_h).pin_memory(), torch.empty_like(u_h).pin_memory()
+    replicas.barrier(dev)
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    load()
+    run.step(K)
+    c, uu, _ = run.fields(False)
+    po.copy_(c, non_blocking=True)
+    uo.copy_(uu, non_blocking=True)
+    t1.record()
+    replicas.barrier(dev)
+    ms_e2e = replicas.max_over_ranks(t0.elapsed_time(t1), dev)
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        b_phase, b_hydro = bytes_per_cell(p.stencil_phase, p.stencil_hydro, esz)
+        step_gbs = (b_phase + b_hydro) * N * K / (ms * 1e-3) / 1e9
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
+               "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": precision, "data": "synthetic",
+               "config": {"workload": name + f", stacked {world}x along z and decomposed into {world} z-slabs",
+                          "grid": [pg.nx, pg.ny, pg.nz], "stencils": [p.stencil_phase, p.stencil_hydro],
+                          "parallelism": f"slab decomposition, {world} rank(s), halo exchange " +
+                                         ("overlapped on a second stream" if run.comm is not None else "in stream order"),
+                          "l2": "inputs larger than L2 (per rank as in the single-GPU run)",
+                          "bytes_per_cell": {"phase": b_phase, "hydro": b_hydro}, "sum_phi_rank0": mass},
+               "clocks": clk.summary(),
+               "e2e": {"value": replicas.aggregate_mlups(N, K, ms_e2e, world), "unit": UNIT, "h2d_bytes_per_step": 4 * N * esz / K,
+                       "d2h_bytes_per_step": 4 * N * esz / K, "steps": K,
+                       "what": "per rank: pinned host phi,u -> device, init, halo exchange, K steps, phi,u -> host"},
+               "gpu_launches": launches,
+               "roofline": {"bound": "hbm", "kernel": "phase + hydro kernels of one rank (whole step, slab schedule)",
+                            "achieved": step_gbs / world, "peak": peak, "unit": "GB/s", "frac": step_gbs / world / peak,
+                            "traffic": None, "peak_source": peak_src}}
+        print(json.dumps(out), flush=True)
+    replicas.shutdown()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -298,12 +382,16 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--inplace", action="store_true", help="in-place AA streaming (one grid per population set)")
     ap.add_argument("--unfused", action="store_true", help="Algorithm 1 (six kernels per step) as a measured comparison")
+    ap.add_argument("--decompose", action="store_true", help="one global domain in z-slabs with halo exchange instead of replicas")
+    ap.add_argument("--no-overlap", action="store_true", help="with --decompose: exchange in stream order (no second stream)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "reference":
         run_reference(args, rank, world)
+    elif args.decompose:
+        run_decomposed(args, rank, local_rank, world)
     else:
         run_acm(args, rank, local_rank, world)
 
