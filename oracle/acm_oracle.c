@@ -113,7 +113,11 @@ static int build_stencil(int Q, lattice_t *L)
     for (int k = 0; k < 27; ++k) {
         int s = abs(DIRS27[k][0]) + abs(DIRS27[k][1]) + abs(DIRS27[k][2]); /* 0 rest,1 axis,2 edge,3 corner */
         double w = -1.0;
-        if (Q == 15) {
+        if (Q == 9) {
+            /* D2Q9: the nine directions of the x-y plane; the grid then has nz = 1 */
+            if (DIRS27[k][2] != 0) continue;
+            if (s == 0) w = 4.0 / 9.0; else if (s == 1) w = 1.0 / 9.0; else w = 1.0 / 36.0;
+        } else if (Q == 15) {
             if (s == 0) w = 2.0 / 9.0; else if (s == 1) w = 1.0 / 9.0; else if (s == 3) w = 1.0 / 72.0;
         } else if (Q == 19) {
             if (s == 0) w = 1.0 / 3.0; else if (s == 1) w = 1.0 / 18.0; else if (s == 2) w = 1.0 / 36.0;
@@ -460,6 +464,9 @@ int oracle_create(oracle_ctx **out, int nx, int ny, int nz, int stencil_phase, i
     if (!o) return 3;
     o->nx = nx; o->ny = ny; o->nz = nz; o->N = (size_t)nx * ny * nz;
     if (build_lattice(stencil_phase, &o->Lh) || build_lattice(stencil_hydro, &o->Lg)) { free(o); return 1; }
+    /* two-dimensional instance: both lattices D2Q9, one plane, no z component of gravity */
+    if ((stencil_phase == 9) != (stencil_hydro == 9)) { free(o); return 1; }
+    if (stencil_phase == 9 && (nz != 1 || (gravity && gravity[2] != 0.0))) { free(o); return 1; }
     o->rho_H = rho_H; o->rho_L = rho_L; o->sigma = sigma; o->xi = xi; o->Mob = Mob; o->nu_H = nu_H; o->nu_L = nu_L;
     for (int a = 0; a < 3; ++a) o->grav[a] = gravity ? gravity[a] : 0.0;
     o->walls = wall_flags;
