@@ -7,7 +7,8 @@ Gram-Schmidt).  The operators follow from the readings A3/A4 of DESIGN.md:
   phase:  Omega^h_ij = delta_ij + (omega_phi - 1) * 3 w_i (e_i . e_j)
           (the w-orthogonal projector on the first-order moments is 3 w_i e_i.e_j)
   hydro:  Omega^g_ij = delta_ij + (s_nu - 1) * 9/2 w_i [ (e_i.e_j)^2 - |e_i|^2/3 - |e_j|^2/3 + 1/3 ]
-          (projector on the six second-order moments x^2-1/3, y^2-1/3, z^2-1/3, xy, xz, yz)
+          (projector on the six second-order moments x^2-1/3, y^2-1/3, z^2-1/3, xy, xz, yz;
+           for D2Q9 the last constant is 2/9: three moments x^2-1/3, y^2-1/3, xy)
 
 Shares nothing with oracle/ or with the CUDA sources; lattices are re-typed here.
 """
@@ -23,7 +24,10 @@ def lattice(Q):
     edge = [(1, 1, 0), (-1, -1, 0), (1, -1, 0), (-1, 1, 0), (1, 0, 1), (-1, 0, -1), (1, 0, -1), (-1, 0, 1),
             (0, 1, 1), (0, -1, -1), (0, 1, -1), (0, -1, 1)]
     corner = [(1, 1, 1), (-1, -1, -1), (1, 1, -1), (-1, -1, 1), (1, -1, 1), (-1, 1, -1), (-1, 1, 1), (1, -1, -1)]
-    if Q == 15:
+    if Q == 9:      # D2Q9: the x-y plane
+        e = [(0, 0, 0)] + axis[:4] + edge[:4]
+        w = [4 / 9] + [1 / 9] * 4 + [1 / 36] * 4
+    elif Q == 15:
         e = [(0, 0, 0)] + axis + corner
         w = [2 / 9] + [1 / 9] * 6 + [1 / 72] * 8
     elif Q == 19:
@@ -149,7 +153,8 @@ def step(par, H, G, C, U, phase_srt=False):
 
         def omega_g(i, j):
             ei, ej = eg[i], eg[j]
-            p2 = dot(ei, ej) ** 2 - dot(ei, ei) / 3.0 - dot(ej, ej) / 3.0 + 1.0 / 3.0
+            # (e_i e_i - I/3) : (e_j e_j - I/3) with I the unit tensor of the lattice's dimension (trace 3, or 2 for D2Q9)
+            p2 = dot(ei, ej) ** 2 - dot(ei, ei) / 3.0 - dot(ej, ej) / 3.0 + (2.0 if Qg == 9 else 3.0) / 9.0
             return (1.0 if i == j else 0.0) + (s - 1.0) * 4.5 * wg[i] * p2
 
         uo = [U[a][zyx] for a in range(3)]
