@@ -49,6 +49,9 @@ def workload(config, size=None):
     elif config == 5:
         p, phi, u = inputs.config5() if size is None else inputs.scaled_config3(size, 27, 27)
         name = f"config5: {p.nx}^3 periodic, seeded bubbles + velocity noise, D3Q27+D3Q27"
+    elif config == 7:
+        p, phi, u = inputs.disc2d() if size is None else inputs.disc2d(n=size, count=4, r_min=size / 16, r_max=size / 8)
+        name = f"2-D instance: {p.nx}^2 periodic, seeded discs + velocity noise, D2Q9+D2Q9 (P:360)"
     elif config == 6:
         p, phi, u = inputs.paper_benchmark() if size is None else inputs.paper_benchmark(n=size)
         name = f"paper benchmark P:283: {p.nx}^3 periodic, one bubble R={p.nx // 4}, D3Q15 SRT + D3Q27 MRT"
@@ -123,7 +126,9 @@ def oracle_sample(config, budget_s, steps=None):
     from oracle import Oracle, oracle as om
     cores = om.set_threads(0)
     # calibrate on 24^3
-    p, phi, u, _ = workload(config if config in (1, 3, 5, 6) else 3, size=24)
+    base = config if config in (1, 3, 5, 6, 7) else 3
+    sz = (lambda n: int(round(n ** 1.5))) if base == 7 else (lambda n: n)      # 2-D: the same number of cells as n^3
+    p, phi, u, _ = workload(base, size=sz(24))
     o = Oracle.from_params(p)
     o.init(phi, u)
     o.step(1)
@@ -139,7 +144,7 @@ def oracle_sample(config, budget_s, steps=None):
         n = 64
         while n > 16 and per_cell * n ** 3 * steps > budget_s:
             n -= 8
-    p, phi, u, name = workload(config if config in (1, 3, 5, 6) else 3, size=n)
+    p, phi, u, name = workload(base, size=sz(n))
     o = Oracle.from_params(p)
     o.init(phi, u)
     t = time.perf_counter()
@@ -172,7 +177,8 @@ def workload_name_only(config):
              3: "config3: 256^3 periodic, seeded bubbles + velocity noise, D3Q15+D3Q19",
              4: "config4: 512^3 periodic, 512 seeded bubbles, D3Q15+D3Q19",
              5: "config5: 256^3 periodic, seeded bubbles + velocity noise, D3Q27+D3Q27",
-             6: "paper benchmark P:283: 260^3 periodic, one bubble R=65, D3Q15 SRT + D3Q27 MRT"}
+             6: "paper benchmark P:283: 260^3 periodic, one bubble R=65, D3Q15 SRT + D3Q27 MRT",
+             7: "2-D instance: 4096^2 periodic, seeded discs + velocity noise, D2Q9+D2Q9 (P:360)"}
     return None, None, None, names[config]
 
 

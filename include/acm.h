@@ -24,6 +24,9 @@
  *     (0,+1,+1)(0,-1,-1)(0,+1,-1)(0,-1,+1); the 8 corner directions
  *     (+1,+1,+1)(-1,-1,-1)(+1,+1,-1)(-1,-1,+1)(+1,-1,+1)(-1,+1,-1)(-1,+1,+1)(+1,-1,-1).
  *     D3Q15 = rest+axis+corner, D3Q19 = rest+axis+edge, D3Q27 = all.
+ *     D2Q9 (the two-dimensional instance the paper measures in Fig. 5) = rest, (+x,-x,+y,-y),
+ *     (+1,+1)(-1,-1)(+1,-1)(-1,+1); it is used for BOTH LB steps on a grid with nz = 1 and gravity[2] = 0;
+ *     u keeps three components, the third stays 0.
  *   - Ownership: the CALLER owns all device memory.  The library never allocates device
  *     memory; acm_create carves the caller's workspace.  The context (host memory) is
  *     freed by acm_destroy only.
@@ -48,7 +51,7 @@ extern "C" {
 typedef struct acm_ctx acm_ctx; /* opaque; owns no device memory */
 
 enum { ACM_OK = 0, ACM_EINVAL = 1, ACM_ESTATE = 2, ACM_ECUDA = 3, ACM_EUNSTABLE = 4 };
-enum { ACM_D3Q15 = 15, ACM_D3Q19 = 19, ACM_D3Q27 = 27 };
+enum { ACM_D2Q9 = 9, ACM_D3Q15 = 15, ACM_D3Q19 = 19, ACM_D3Q27 = 27 };
 /* set: half-way bounce-back no-slip walls on both faces of that axis; clear: periodic */
 enum { ACM_WALL_X = 1, ACM_WALL_Y = 2, ACM_WALL_Z = 4 };
 enum { ACM_F64 = 0, ACM_F32 = 1 };
@@ -60,7 +63,7 @@ size_t acm_workspace_bytes(int nx, int ny, int nz, int stencil_phase, int stenci
 
 /* Creates a context.  Parameters follow the paper's statement of the problem:
  *   nx,ny,nz        grid size in cells (each >= 1; nx*ny*nz < 2^31)
- *   stencil_phase   lattice of h: ACM_D3Q15 | ACM_D3Q19 | ACM_D3Q27
+ *   stencil_phase   lattice of h: ACM_D3Q15 | ACM_D3Q19 | ACM_D3Q27, or ACM_D2Q9 for both
  *   stencil_hydro   lattice of g: ACM_D3Q19 | ACM_D3Q27 (ACM_D3Q15 also accepted)
  *   rho_H, rho_L    densities of the heavy / light phase, rho_H >= rho_L > 0   (eq. 8)
  *   sigma           surface tension >= 0; beta = 12 sigma/xi, kappa = 3 sigma xi/2

@@ -62,7 +62,7 @@ struct acm_ctx {
 
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
-static bool valid_stencil(int q) { return q == 15 || q == 19 || q == 27; }
+static bool valid_stencil(int q) { return q == 9 || q == 15 || q == 19 || q == 27; }
 
 struct Layout {
     size_t offH[2], offG[2], offC[2], offU[2], offStage, offRed, total;
@@ -74,6 +74,7 @@ static bool make_layout(int nx, int ny, int nz, int Qh, int Qg, int precision, u
     if ((options & ACM_OPT_UNFUSED) && (options & ACM_OPT_INPLACE)) return false;   // Algorithm 1 is a two-grid scheme
     const int grids = (options & ACM_OPT_INPLACE) ? 1 : 2;
     if (nx <= 0 || ny <= 0 || nz <= 0 || !valid_stencil(Qh) || !valid_stencil(Qg)) return false;
+    if ((Qh == 9) != (Qg == 9)) return false;      // the two-dimensional instance uses D2Q9 for both LB steps
     if (precision != ACM_F64 && precision != ACM_F32) return false;
     const double cells = (double)nx * ny * nz;
     if (cells >= 2147483648.0) return false;
@@ -319,6 +320,8 @@ static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase,
     if (!(M > 0.0) || !std::isfinite(M)) return fail(ACM_EINVAL, "acm_create: need mobility M > 0");
     if (!(nu_H > 0.0) || !(nu_L > 0.0)) return fail(ACM_EINVAL, "acm_create: need nu_H, nu_L > 0");
     if (wall_flags & ~7u) return fail(ACM_EINVAL, "acm_create: unknown wall flag");
+    if (stencil_phase == 9 && (nzl != 1 || slab || (gravity && gravity[2] != 0.0)))
+        return fail(ACM_EINVAL, "acm_create: D2Q9 needs nz = 1, no slab decomposition and gravity[2] = 0");
     if (!workspace) return fail(ACM_EINVAL, "acm_create: workspace is NULL");
     if ((uintptr_t)workspace & 255) return fail(ACM_EINVAL, "acm_create: workspace must be 256-byte aligned");
     acm_ctx* c = new (std::nothrow) acm_ctx();
@@ -428,7 +431,7 @@ static int crossing_dirs(int Q, int sign, int* dirs)
 {
     int n = 0;
     for (int i = 0; i < Q; ++i) {
-        const int k = (Q == 15 && i >= 7) ? i + 12 : i;
+        const int k = (Q == 15 && i >= 7) ? i + 12 : (Q == 9 && i >= 5) ? i + 2 : i;
         if (acm::dir27(k, 2) == sign) dirs[n++] = i;
     }
     return n;

@@ -181,6 +181,14 @@ __global__ void __launch_bounds__(RED_THREADS) diag_pass2(const double* __restri
 // ------------------------------------------------------------------------------------------
 #define ACM_DISPATCH_Q(q, QQ, ...)                                 \
     switch (q) {                                                    \
+        case 9: { constexpr int QQ = 9; __VA_ARGS__; } break;       \
+        case 15: { constexpr int QQ = 15; __VA_ARGS__; } break;     \
+        case 19: { constexpr int QQ = 19; __VA_ARGS__; } break;     \
+        default: { constexpr int QQ = 27; __VA_ARGS__; } break;     \
+    }
+
+#define ACM_DISPATCH_Q3(q, QQ, ...)                                \
+    switch (q) {                                                    \
         case 15: { constexpr int QQ = 15; __VA_ARGS__; } break;     \
         case 19: { constexpr int QQ = 19; __VA_ARGS__; } break;     \
         default: { constexpr int QQ = 27; __VA_ARGS__; } break;     \
@@ -189,7 +197,12 @@ __global__ void __launch_bounds__(RED_THREADS) diag_pass2(const double* __restri
 template <typename T>
 cudaError_t launch_init(int Qh, int Qg, bool inplace, const Launch& l, const T* phi, const T* u, T* H, T* G, T* C, T* U, Geom g, size_t N)
 {
-    ACM_DISPATCH_Q(Qh, QH, ACM_DISPATCH_Q(Qg, QG, {
+    if (Qh == 9 || Qg == 9) {       // the two-dimensional instance uses D2Q9 for both steps
+        if (inplace) init_kernel<T, 9, 9, true><<<l.grid, l.block, 0, l.stream>>>(phi, u, H, G, C, U, g, N);
+        else init_kernel<T, 9, 9, false><<<l.grid, l.block, 0, l.stream>>>(phi, u, H, G, C, U, g, N);
+        return cudaGetLastError();
+    }
+    ACM_DISPATCH_Q3(Qh, QH, ACM_DISPATCH_Q3(Qg, QG, {
         if (inplace) init_kernel<T, QH, QG, true><<<l.grid, l.block, 0, l.stream>>>(phi, u, H, G, C, U, g, N);
         else init_kernel<T, QH, QG, false><<<l.grid, l.block, 0, l.stream>>>(phi, u, H, G, C, U, g, N);
     }));

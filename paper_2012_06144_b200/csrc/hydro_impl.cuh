@@ -57,7 +57,8 @@ static void launch_hydro_q(bool walls, int state, const Launch& l, const HydroAr
 template <typename T>
 cudaError_t launch_hydro(int Q, bool walls, int state, const Launch& l, const HydroArgs<T>& a)
 {
-    if (Q == 15) launch_hydro_q<T, 15>(walls, state, l, a);
+    if (Q == 9) launch_hydro_q<T, 9>(walls, state, l, a);
+    else if (Q == 15) launch_hydro_q<T, 15>(walls, state, l, a);
     else if (Q == 19) launch_hydro_q<T, 19>(walls, state, l, a);
     else launch_hydro_q<T, 27>(walls, state, l, a);
     return cudaGetLastError();

@@ -1,4 +1,4 @@
-// lattice.cuh -- compile-time D3Q15/D3Q19/D3Q27 tables and the two shared "moment <-> population"
+// lattice.cuh -- compile-time D2Q9/D3Q15/D3Q19/D3Q27 tables and the two shared "moment <-> population"
 // building blocks of the ACM kernels (no runtime tables: everything folds into immediates).
 //
 // Canonical direction order (include/acm.h): rest; axis pairs; edge pairs; corner pairs; the
@@ -24,9 +24,11 @@ __host__ __device__ constexpr int dir27(int k, int a)
 
 template <int Q>
 struct Lat {
-    static_assert(Q == 15 || Q == 19 || Q == 27, "unsupported lattice");
+    static_assert(Q == 9 || Q == 15 || Q == 19 || Q == 27, "unsupported lattice");
+    // D2Q9: the nine directions of the x-y plane, on a grid with one z plane
+    static constexpr int DIM = Q == 9 ? 2 : 3;
     // index into the 27-direction list
-    __host__ __device__ static constexpr int k27(int i) { return (Q == 15 && i >= 7) ? i + 12 : i; }
+    __host__ __device__ static constexpr int k27(int i) { return (Q == 15 && i >= 7) ? i + 12 : (Q == 9 && i >= 5) ? i + 2 : i; }
     __host__ __device__ static constexpr int ex(int i) { return dir27(k27(i), 0); }
     __host__ __device__ static constexpr int ey(int i) { return dir27(k27(i), 1); }
     __host__ __device__ static constexpr int ez(int i) { return dir27(k27(i), 2); }
@@ -36,12 +38,13 @@ struct Lat {
     // weight of a class
     __host__ __device__ static constexpr double wc(int c)
     {
-        return Q == 15 ? (c == 0 ? 2.0 / 9.0 : c == 1 ? 1.0 / 9.0 : 1.0 / 72.0)
+        return Q == 9  ? (c == 0 ? 4.0 / 9.0 : c == 1 ? 1.0 / 9.0 : 1.0 / 36.0)
+             : Q == 15 ? (c == 0 ? 2.0 / 9.0 : c == 1 ? 1.0 / 9.0 : 1.0 / 72.0)
              : Q == 19 ? (c == 0 ? 1.0 / 3.0 : c == 1 ? 1.0 / 18.0 : 1.0 / 36.0)
                        : (c == 0 ? 8.0 / 27.0 : c == 1 ? 2.0 / 27.0 : c == 2 ? 1.0 / 54.0 : 1.0 / 216.0);
     }
     __host__ __device__ static constexpr double w(int i) { return wc(cls(i)); }
-    __host__ __device__ static constexpr bool has_cls(int c) { return c <= 1 || (c == 2 && Q != 15) || (c == 3 && Q != 19); }
+    __host__ __device__ static constexpr bool has_cls(int c) { return c <= 1 || (c == 2 && Q != 15) || (c == 3 && Q != 19 && Q != 9); }
 };
 
 template <int I, int N, int S = 1, typename F>

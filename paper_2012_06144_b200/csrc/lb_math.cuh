@@ -131,7 +131,9 @@ __device__ __forceinline__ void hydro_collide(const Moments<Q, T, true>& m, cons
     const T Txy = s45 * ux * uy + k45 * (m.Pxy - ux * uy);
     const T Txz = s45 * ux * uz + k45 * (m.Pxz - ux * uz);
     const T Tyz = s45 * uy * uz + k45 * (m.Pyz - uy * uz);
-    const T A = pstar - T(1.5) * (ux * ux + uy * uy + uz * uz) - T(1.5) * om * (nxx + nyy + nzz);
+    // trace of Pi over the lattice's dimensions (D2Q9: the plane only; u_z = 0 there)
+    const T trPi = Lat<Q>::DIM == 3 ? nxx + nyy + nzz : nxx + nyy;
+    const T A = pstar - T(1.5) * (ux * ux + uy * uy + uz * uz) - T(1.5) * om * trPi;
     const T bx = T(3) * (ux + hx), by = T(3) * (uy + hy), bz = T(3) * (uz + hz);
     emit_populations<Q, T>(A, bx, by, bz, Txx, Tyy, Tzz, Txy, Txz, Tyz, store);
 }

@@ -63,7 +63,8 @@ static void launch_phase_q(bool walls, int state, int collision, const Launch& l
 template <typename T>
 cudaError_t launch_phase(int Q, bool walls, int state, int collision, const Launch& l, const PhaseArgs<T>& a)
 {
-    if (Q == 15) launch_phase_q<T, 15>(walls, state, collision, l, a);
+    if (Q == 9) launch_phase_q<T, 9>(walls, state, collision, l, a);
+    else if (Q == 15) launch_phase_q<T, 15>(walls, state, collision, l, a);
     else if (Q == 19) launch_phase_q<T, 19>(walls, state, collision, l, a);
     else launch_phase_q<T, 27>(walls, state, collision, l, a);
     return cudaGetLastError();

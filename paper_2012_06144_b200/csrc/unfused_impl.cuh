@@ -139,6 +139,7 @@ static cudaError_t unfused_hydro_qw(const Launch& l, const HydroArgs<T>& a, cons
 template <typename T>
 cudaError_t launch_unfused_phase(int Q, bool walls, int collision, const Launch& l, const PhaseArgs<T>& a)
 {
+    if (Q == 9) return walls ? unfused_phase_qw<T, 9, true>(collision, l, a) : unfused_phase_qw<T, 9, false>(collision, l, a);
     if (Q == 15) return walls ? unfused_phase_qw<T, 15, true>(collision, l, a) : unfused_phase_qw<T, 15, false>(collision, l, a);
     if (Q == 19) return walls ? unfused_phase_qw<T, 19, true>(collision, l, a) : unfused_phase_qw<T, 19, false>(collision, l, a);
     return walls ? unfused_phase_qw<T, 27, true>(collision, l, a) : unfused_phase_qw<T, 27, false>(collision, l, a);
@@ -147,6 +148,7 @@ cudaError_t launch_unfused_phase(int Q, bool walls, int collision, const Launch&
 template <typename T>
 cudaError_t launch_unfused_hydro(int Q, bool walls, const Launch& l, const HydroArgs<T>& a, const T* Uold, T* Unew)
 {
+    if (Q == 9) return walls ? unfused_hydro_qw<T, 9, true>(l, a, Uold, Unew) : unfused_hydro_qw<T, 9, false>(l, a, Uold, Unew);
     if (Q == 15) return walls ? unfused_hydro_qw<T, 15, true>(l, a, Uold, Unew) : unfused_hydro_qw<T, 15, false>(l, a, Uold, Unew);
     if (Q == 19) return walls ? unfused_hydro_qw<T, 19, true>(l, a, Uold, Unew) : unfused_hydro_qw<T, 19, false>(l, a, Uold, Unew);
     return walls ? unfused_hydro_qw<T, 27, true>(l, a, Uold, Unew) : unfused_hydro_qw<T, 27, false>(l, a, Uold, Unew);

@@ -208,6 +208,26 @@ def paper_benchmark(n: int = 260, R: Optional[float] = None):
     return p, phi, zeros_u(p)
 
 
+def disc2d(n: int = 4096, count: int = 64, r_min: float = 40.0, r_max: float = 80.0, noise: float = 1.0e-3):
+    """Two-dimensional instance (D2Q9 + D2Q9, one plane; the paper's Fig. 5 measures D2Q9): seeded light
+    discs in heavy liquid on an n x n periodic grid, same recipe as config 3 (centres in the plane z = 1/2)."""
+    p = Params(nx=n, ny=n, nz=1, stencil_phase=9, stencil_hydro=9)
+    rng = np.random.Generator(np.random.PCG64(SEED_BUBBLES))
+    centres, radii = [], []
+    while len(centres) < count:
+        c = np.array([rng.uniform(0, n), rng.uniform(0, n), 0.5])
+        R = rng.uniform(r_min, r_max)
+        d = np.abs(np.array(centres).reshape(-1, 3) - c)[:, :2] if centres else np.zeros((0, 2))
+        d = np.minimum(d, n - d)
+        if all(np.sqrt((d * d).sum(1)) >= R + np.array(radii) + 2.0 * p.xi):
+            centres.append(c)
+            radii.append(R)
+    phi = bubbles_phi(p, np.array(centres), np.array(radii))
+    u = velocity_noise(p, noise) if noise > 0 else zeros_u(p)
+    u[2] = 0.0
+    return p, phi, u
+
+
 def scaled_config3(n: int, stencil_phase: int = 15, stencil_hydro: int = 19):
     """Config-3-like input on a small grid: bubble count and radii scaled so that
     the volume fraction and the interface structure stay comparable."""
