@@ -113,6 +113,15 @@ int acm_create_opt(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int
  * (eq. 12 with p* = 0).  phi: [device] N values; u: [device] 3N values, component-major. */
 int acm_init(acm_ctx*, const void* phi, const void* u);
 
+/* ACM_F32 only (no effect for ACM_F64).  The fp32 instance stores h_i - ref w_i and phi - ref instead of h_i and
+ * phi, where ref = 0 (light) or 1 (heavy) is a reference phase: the bulk of that phase then keeps all its digits
+ * (phi = 1 - 1e-4 has 3 significant digits left in fp32, its deviation -1e-4 has 7), which matters because the
+ * interface normal of eq. 5 is taken from differences of phi.  Same idea as the velocity-based g of the paper,
+ * which already carries g_i - w_i (eq. 12).  phase = -1 (default): acm_init takes the phase that fills most of the
+ * domain (the heavy one for slabs, which must all agree); 0 / 1 force it.  Arrays crossing the ABI are unaffected.
+ * ACM_ESTATE after acm_init. */
+int acm_set_reference_phase(acm_ctx*, int phase);
+
 /* Advances n >= 0 time steps (phase-field kernel, then hydrodynamic kernel, per step).
  * Asynchronous.  ACM_ESTATE before acm_init. */
 int acm_step(acm_ctx*, int n);

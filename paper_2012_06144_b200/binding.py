@@ -18,7 +18,7 @@ ACM_WALL_X, ACM_WALL_Y, ACM_WALL_Z = 1, 2, 4
 ACM_OPT_INPLACE, ACM_OPT_PHASE_SRT, ACM_OPT_UNFUSED = 1, 2, 4
 
 EXPORTS = ["acm_workspace_bytes", "acm_workspace_bytes_opt", "acm_create", "acm_create_opt", "acm_init", "acm_step", "acm_fields", "acm_phi_mass", "acm_get_pdfs",
-           "acm_set_pdfs", "acm_run_host", "acm_bubble_diag", "acm_bubble_sums", "acm_slab_range", "acm_workspace_bytes_slab", "acm_create_slab", "acm_slab_info",
+           "acm_set_pdfs", "acm_run_host", "acm_set_reference_phase", "acm_bubble_diag", "acm_bubble_sums", "acm_slab_range", "acm_workspace_bytes_slab", "acm_create_slab", "acm_slab_info",
            "acm_halo_plan", "acm_phase_launch", "acm_phase_commit", "acm_hydro_launch", "acm_hydro_commit", "acm_bubble_params", "acm_drag_lbm", "acm_drag_exp", "acm_set_block", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
 
 _lib = None
@@ -61,6 +61,7 @@ def load(build_if_missing: bool = True):
     lib.acm_set_pdfs.argtypes = [vp, vp, vp]
     lib.acm_run_host.argtypes = [vp, vp, vp, i32, vp, vp, vp]
     lib.acm_bubble_diag.argtypes = [vp, C.POINTER(dbl)]
+    lib.acm_set_reference_phase.argtypes = [vp, i32]
     lib.acm_bubble_sums.argtypes = [vp, C.POINTER(dbl)]
     lib.acm_slab_range.argtypes = [i32, i32, i32, C.POINTER(i32), C.POINTER(i32)]
     lib.acm_workspace_bytes_slab.restype = C.c_size_t
@@ -172,6 +173,10 @@ class ACM:
 
     def set_block(self, bx, by=1, bz=1):
         self._call(self._lib.acm_set_block, int(bx), int(by), int(bz))
+
+    def set_reference_phase(self, phase):
+        """fp32 instance: reference phase of the deviation storage (-1 automatic, 0 light, 1 heavy); before init"""
+        self._call(self._lib.acm_set_reference_phase, int(phase))
 
     def init(self, phi, u):
         self._call(self._lib.acm_init, self._dev(phi, self.shape), self._dev(u, (3,) + self.shape))

@@ -41,6 +41,9 @@ struct acm_ctx {
     // slab of a z-decomposed domain (acm_create_slab); a plain context owns everything: nzl = nz, zlo = 0
     int nzl, zlo, ghost;                  // owned planes [zlo, zlo+nzl), ghost = 1: planes zlo-1 and zlo+nzl are halos
     int zglob0, nz_global, rank, nranks;  // global z of the first owned plane, global height, position in the decomposition
+    // fp32 instance: h and phi are stored as deviations from the reference phase (A22)
+    int ref_mode;                         // -1: chosen by acm_init (the majority phase; heavy for slabs), else 0 / 1
+    double ref;                           // 0 or 1; always 0 for fp64
     double rho_H, rho_L, sigma, xi, M, nu_H, nu_L, grav[3];
     unsigned walls;
     cudaStream_t stream;
@@ -142,7 +145,7 @@ static int init_t(acm_ctx* c, const void* phi, const void* u)
     const bool inplace = (c->options & ACM_OPT_INPLACE) != 0;
     T *H = wsp<T>(c, c->offH[0]), *G = wsp<T>(c, c->offG[0]), *C = wsp<T>(c, c->offC[0]), *U = wsp<T>(c, c->offU[0]);
     cudaError_t e = launch_init<T>(c->Qh, c->Qg, inplace, aux_launch(c), (const T*)phi, (const T*)u, H, G, C, U,
-                                   geom_of(c), c->N);
+                                   geom_of(c), c->N, (T)c->ref);
     if (inplace) { c->stH = ST_SWAP; c->stG = ST_IN; }
     else c->stH = c->stG = ST_POST;
     c->curH = c->curG = c->curC = c->curU = 0;
@@ -167,6 +170,7 @@ static int launch_phase_range(acm_ctx* c, int z0, int z1)
     const double omega = 1.0 / (3.0 * c->M + 0.5);     // tau_phi = M/c_s^2 (eq. 2), shifted by 1/2
     a.one_minus_omega = (T)(1.0 - omega);
     a.inv_xi = (T)(1.0 / c->xi);
+    a.ref = (T)c->ref;
     const Launch l = lb_launch(c, z1 - z0);
     const int coll = (c->options & ACM_OPT_PHASE_SRT) ? PHASE_SRT : PHASE_MRT;
     const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
@@ -191,8 +195,10 @@ static int launch_hydro_range(acm_ctx* c, int z0, int z1)
     a.U = wsp<T>(c, c->offU[c->curU]);
     a.g = geom_of(c, lb_linear(c), z0, z1);
     a.N = c->N;
-    a.rho_L = (T)c->rho_L; a.drho = (T)(c->rho_H - c->rho_L);
-    a.tau_L = (T)(3.0 * c->nu_L); a.dtau = (T)(3.0 * c->nu_H - 3.0 * c->nu_L);
+    // rho and tau at the reference phase of the stored phi (ref = 0: the light phase, as in eqs. 8, 20)
+    a.ref = (T)c->ref;
+    a.rho_L = (T)(c->rho_L + c->ref * (c->rho_H - c->rho_L)); a.drho = (T)(c->rho_H - c->rho_L);
+    a.tau_L = (T)(3.0 * c->nu_L + c->ref * (3.0 * c->nu_H - 3.0 * c->nu_L)); a.dtau = (T)(3.0 * c->nu_H - 3.0 * c->nu_L);
     a.beta4 = (T)(4.0 * 12.0 * c->sigma / c->xi); a.kappa = (T)(1.5 * c->sigma * c->xi);
     a.gx = (T)c->grav[0]; a.gy = (T)c->grav[1]; a.gz = (T)c->grav[2];
     const Launch l = lb_launch(c, z1 - z0);
@@ -253,7 +259,7 @@ template <typename T>
 static int export_g_t(acm_ctx* c, void* g, void* p)      // incoming convention (+ pressure)
 {
     cudaError_t e = launch_export<T>(c->Qg, c->stG, false, aux_launch(c), wsp<T>(c, c->offG[c->curG]), wsp<T>(c, c->offC[c->curC]),
-                                     (T*)g, (T*)p, geom_of(c), c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L));
+                                     (T*)g, (T*)p, geom_of(c), c->N, (T)(c->rho_L + c->ref * (c->rho_H - c->rho_L)), (T)(c->rho_H - c->rho_L), (T)0);
     return check_launch(c, "export_kernel", e);
 }
 
@@ -261,7 +267,7 @@ template <typename T>
 static int export_h_t(acm_ctx* c, void* h)               // post-collision convention
 {
     cudaError_t e = launch_export<T>(c->Qh, c->stH, true, aux_launch(c), wsp<T>(c, c->offH[c->curH]), wsp<T>(c, c->offC[c->curC]),
-                                     (T*)h, (T*)nullptr, geom_of(c), c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L));
+                                     (T*)h, (T*)nullptr, geom_of(c), c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L), (T)c->ref);
     return check_launch(c, "export_kernel", e);
 }
 
@@ -269,7 +275,7 @@ template <typename T>
 static int import_g_t(acm_ctx* c, const void* g)      // incoming convention -> ST_POST storage
 {
     cudaError_t e = launch_import<T>(c->Qg, false, aux_launch(c), (const T*)g, wsp<T>(c, c->offG[c->curG]),
-                                     geom_of(c), c->N);
+                                     geom_of(c), c->N, (T)0);
     return check_launch(c, "import_kernel", e);
 }
 
@@ -277,7 +283,7 @@ template <typename T>
 static int import_h_t(acm_ctx* c, const void* h)      // post-collision convention -> ST_SWAP storage
 {
     cudaError_t e = launch_import<T>(c->Qh, true, aux_launch(c), (const T*)h, wsp<T>(c, c->offH[c->curH]),
-                                     geom_of(c), c->N);
+                                     geom_of(c), c->N, (T)c->ref);
     return check_launch(c, "import_kernel", e);
 }
 
@@ -289,6 +295,15 @@ static int copy_async(acm_ctx* c, void* dst, const void* src, size_t bytes, cuda
         return fail(ACM_ECUDA, "%s: %s", what, cudaGetErrorString(e));
     }
     return ACM_OK;
+}
+
+// dst = phi-field-like source + shift (device to device); a plain copy when shift = 0
+static int copy_field_shifted(acm_ctx* c, void* dst, const void* src, size_t n, double shift, const char* what)
+{
+    if (shift == 0.0) return copy_async(c, dst, src, n * c->esz, cudaMemcpyDeviceToDevice, what);
+    cudaError_t e = c->precision == ACM_F64 ? launch_shift_field<double>(c->stream, (const double*)src, (double*)dst, n, shift)
+                                            : launch_shift_field<float>(c->stream, (const float*)src, (float*)dst, n, (float)shift);
+    return check_launch(c, what, e);
 }
 
 #define ACM_CHECK_CTX(c)                                                          \
@@ -336,6 +351,7 @@ static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase,
         if (!slab || rank == 0) c->walls |= WALL_ZLO;
         if (!slab || rank == nranks - 1) c->walls |= WALL_ZHI;
     }
+    c->ref_mode = -1; c->ref = 0.0;
     c->nzl = nzl; c->zlo = slab ? 1 : 0; c->ghost = slab ? 1 : 0;
     c->zglob0 = zglob0; c->nz_global = slab ? nz_global : nzl; c->rank = slab ? rank : 0; c->nranks = slab ? nranks : 1;
     c->stream = (cudaStream_t)cuda_stream;
@@ -563,17 +579,42 @@ int acm_init(acm_ctx* c, const void* phi, const void* u)
 {
     ACM_CHECK_CTX(c);
     if (!phi || !u) return fail(ACM_EINVAL, "acm_init: phi and u are required");
+    c->ref = 0.0;
+    if (c->precision == ACM_F32) {
+        // reference phase of the deviation storage: the phase that fills most of the domain
+        if (c->ref_mode >= 0) c->ref = c->ref_mode;
+        else if (c->ghost) c->ref = 1.0;      // every slab of a decomposition must take the same one: bubbles in liquid
+        else {
+            double* part = wsp<double>(c, c->offRed);
+            double total = 0.0;
+            int rc0 = check_launch(c, "sum_phi", launch_sum_phi<float>(c->stream, (const float*)phi, c->N, part), 2);
+            if (!rc0) rc0 = copy_async(c, &total, part + RED_BLOCKS, sizeof(double), cudaMemcpyDeviceToHost, "acm_init(mean phi)");
+            if (rc0) return rc0;
+            if (cudaStreamSynchronize(c->stream) != cudaSuccess) { c->sticky = ACM_ECUDA; return fail(ACM_ECUDA, "acm_init: synchronize failed"); }
+            c->ref = total > 0.5 * (double)c->N ? 1.0 : 0.0;
+        }
+    }
     int rc = c->precision == ACM_F64 ? init_t<double>(c, phi, u) : init_t<float>(c, phi, u);
     if (rc == ACM_OK && c->ghost) {
         // slab: phi and u come with their ghost planes filled (the pre-shifted g needs u of the neighbour planes);
         // the phi ghost planes are taken over as they are, those of h and g arrive with the first halo exchange
         const size_t plane = (size_t)c->nx * c->ny * c->esz;
         const size_t hi = (size_t)(c->zlo + c->nzl) * plane;
-        rc = copy_async(c, c->ws + c->offC[0], phi, plane, cudaMemcpyDeviceToDevice, "acm_init(phi ghost)");
-        if (!rc) rc = copy_async(c, c->ws + c->offC[0] + hi, (const char*)phi + hi, plane, cudaMemcpyDeviceToDevice, "acm_init(phi ghost)");
+        const size_t cells = (size_t)c->nx * c->ny;
+        rc = copy_field_shifted(c, c->ws + c->offC[0], phi, cells, -c->ref, "acm_init(phi ghost)");
+        if (!rc) rc = copy_field_shifted(c, c->ws + c->offC[0] + hi, (const char*)phi + hi, cells, -c->ref, "acm_init(phi ghost)");
     }
     if (rc == ACM_OK) c->initialised = true;
     return rc;
+}
+
+int acm_set_reference_phase(acm_ctx* c, int phase)
+{
+    ACM_CHECK_CTX(c);
+    if (phase < -1 || phase > 1) return fail(ACM_EINVAL, "acm_set_reference_phase: phase must be -1 (automatic), 0 (light) or 1 (heavy)");
+    if (c->initialised) return fail(ACM_ESTATE, "acm_set_reference_phase: must be called before acm_init");
+    c->ref_mode = phase;
+    return ACM_OK;
 }
 
 int acm_step(acm_ctx* c, int n)
@@ -590,7 +631,7 @@ int acm_fields(acm_ctx* c, void* phi, void* u, void* p)
     ACM_CHECK_CTX(c);
     if (!c->initialised) return fail(ACM_ESTATE, "acm_fields: call acm_init first");
     int rc = ACM_OK;
-    if (phi) rc = copy_async(c, phi, c->ws + c->offC[c->curC], c->N * c->esz, cudaMemcpyDeviceToDevice, "acm_fields(phi)");
+    if (phi) rc = copy_field_shifted(c, phi, c->ws + c->offC[c->curC], c->N, c->ref, "acm_fields(phi)");
     if (!rc && u) rc = copy_async(c, u, c->ws + c->offU[c->curU], 3 * c->N * c->esz, cudaMemcpyDeviceToDevice, "acm_fields(u)");
     if (!rc && p) rc = c->precision == ACM_F64 ? export_g_t<double>(c, nullptr, p) : export_g_t<float>(c, nullptr, p);
     return rc;
@@ -611,6 +652,7 @@ int acm_phi_mass(acm_ctx* c, double* total_host)
     if (rc) return rc;
     cudaError_t e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) { c->sticky = ACM_ECUDA; return fail(ACM_ECUDA, "acm_phi_mass: %s", cudaGetErrorString(e)); }
+    *total_host += c->ref * (double)owned;        // fp32 instance: the field holds phi - ref
     if (!std::isfinite(*total_host)) return fail(ACM_EUNSTABLE, "acm_phi_mass: sum(phi) is not finite");
     return ACM_OK;
 }
@@ -624,8 +666,8 @@ int acm_bubble_sums(acm_ctx* c, double out_host[7])
     const Geom g = geom_of(c);
     const int zshift = c->zglob0 - c->zlo;
     cudaError_t le = c->precision == ACM_F64
-                         ? launch_bubble_diag<double>(c->stream, wsp<double>(c, c->offC[c->curC]), wsp<double>(c, c->offU[c->curU]), g, c->N, zshift, part)
-                         : launch_bubble_diag<float>(c->stream, wsp<float>(c, c->offC[c->curC]), wsp<float>(c, c->offU[c->curU]), g, c->N, zshift, part);
+                         ? launch_bubble_diag<double>(c->stream, wsp<double>(c, c->offC[c->curC]), wsp<double>(c, c->offU[c->curU]), g, c->N, zshift, c->ref, part)
+                         : launch_bubble_diag<float>(c->stream, wsp<float>(c, c->offC[c->curC]), wsp<float>(c, c->offU[c->curU]), g, c->N, zshift, c->ref, part);
     int rc = check_launch(c, "bubble_diag", le, 2);
     if (rc) return rc;
     rc = copy_async(c, out_host, part + (size_t)DIAG_WIDTH * RED_BLOCKS, DIAG_WIDTH * sizeof(double), cudaMemcpyDeviceToHost, "acm_bubble_sums");
@@ -695,7 +737,8 @@ int acm_set_pdfs(acm_ctx* c, const void* h, const void* g)
     if (h) {
         // post-collision convention: two-grid stores it as is (ST_POST); in place as ST_SWAP
         if (inplace) { rc = c->precision == ACM_F64 ? import_h_t<double>(c, h) : import_h_t<float>(c, h); c->stH = ST_SWAP; }
-        else rc = copy_async(c, c->ws + c->offH[c->curH], h, (size_t)c->Qh * c->N * c->esz, cudaMemcpyDeviceToDevice, "acm_set_pdfs(h)");
+        else if (c->ref == 0.0) rc = copy_async(c, c->ws + c->offH[c->curH], h, (size_t)c->Qh * c->N * c->esz, cudaMemcpyDeviceToDevice, "acm_set_pdfs(h)");
+        else rc = check_launch(c, "shift_pop_kernel", launch_shift_pop<float>(c->Qh, aux_launch(c), (const float*)h, wsp<float>(c, c->offH[c->curH]), geom_of(c), c->N, (float)-c->ref));
     }
     if (!rc && g) {
         // incoming convention: in place stores it as is (ST_IN); two-grid pre-shifts it into ST_POST
@@ -719,7 +762,14 @@ int acm_run_host(acm_ctx* c, const void* phi_host, const void* u_host, int n, vo
     if (!rc) rc = acm_init(c, st, st + fb);
     if (!rc) rc = acm_step(c, n);
     if (!rc && p_out_host) rc = acm_fields(c, nullptr, nullptr, st + 4 * fb);
-    if (!rc && phi_out_host) rc = copy_async(c, phi_out_host, c->ws + c->offC[c->curC], fb, cudaMemcpyDeviceToHost, "acm_run_host(d2h phi)");
+    if (!rc && phi_out_host) {
+        const char* src = c->ws + c->offC[c->curC];
+        if (c->ref != 0.0) {      // un-shift phi into the staging area first (its phi/u slots are free after acm_init)
+            rc = copy_field_shifted(c, st, src, c->N, c->ref, "acm_run_host(phi)");
+            src = st;
+        }
+        if (!rc) rc = copy_async(c, phi_out_host, src, fb, cudaMemcpyDeviceToHost, "acm_run_host(d2h phi)");
+    }
     if (!rc && u_out_host) rc = copy_async(c, u_out_host, c->ws + c->offU[c->curU], 3 * fb, cudaMemcpyDeviceToHost, "acm_run_host(d2h u)");
     if (!rc && p_out_host) rc = copy_async(c, p_out_host, st + 4 * fb, fb, cudaMemcpyDeviceToHost, "acm_run_host(d2h p)");
     if (rc) return rc;

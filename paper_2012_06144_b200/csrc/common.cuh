@@ -248,6 +248,7 @@ struct PhaseArgs {
     Geom g;
     size_t N;
     T one_minus_omega, inv_xi;
+    T ref;           // fp32 instance: reference phase of the deviation storage (0 or 1); 0 for fp64
 };
 
 template <typename T>
@@ -258,6 +259,7 @@ struct HydroArgs {
     Geom g;
     size_t N;
     T rho_L, drho, tau_L, dtau, beta4, kappa, gx, gy, gz;
+    T ref;           // as in PhaseArgs; rho_L, tau_L are the values at phi = ref
 };
 
 }  // namespace acm

@@ -25,13 +25,16 @@ template <typename T> cudaError_t launch_unfused_hydro(int Q, bool walls, const 
 
 // Equilibrium initialiser.
 template <typename T>
-cudaError_t launch_init(int Qh, int Qg, bool inplace, const Launch& l, const T* phi, const T* u, T* H, T* G, T* C, T* U, Geom g, size_t N);
+cudaError_t launch_init(int Qh, int Qg, bool inplace, const Launch& l, const T* phi, const T* u, T* H, T* G, T* C, T* U, Geom g, size_t N, T ref);
 // Export of a population array stored in `state` in the POST (post-collision at own cell) or
 // incoming convention; optionally the pressure p = c_s^2 rho(phi) sum_i f_i.
 template <typename T>
-cudaError_t launch_export(int Q, int state, bool post, const Launch& l, const T* F, const T* C, T* out, T* p, Geom g, size_t N, T rho_L, T drho);
+cudaError_t launch_export(int Q, int state, bool post, const Launch& l, const T* F, const T* C, T* out, T* p, Geom g, size_t N, T rho_L, T drho, T shift);
 // Import: POST convention -> ST_SWAP storage, or incoming convention -> ST_POST storage.
-template <typename T> cudaError_t launch_import(int Q, bool post, const Launch& l, const T* in, T* F, Geom g, size_t N);
+template <typename T> cudaError_t launch_import(int Q, bool post, const Launch& l, const T* in, T* F, Geom g, size_t N, T shift);
+// fp32 deviation storage (A22): out_i = in_i + shift w_i on the owned cells; out = in + shift on a whole field.
+template <typename T> cudaError_t launch_shift_pop(int Q, const Launch& l, const T* in, T* out, Geom g, size_t N, T shift);
+template <typename T> cudaError_t launch_shift_field(cudaStream_t s, const T* in, T* out, size_t n, T shift);
 
 // Deterministic two-pass reductions.  `part` holds RED_BLOCKS * width partial sums followed by
 // `width` results.
@@ -39,6 +42,6 @@ constexpr int RED_BLOCKS = 592, RED_THREADS = 256;   // 4 CTAs per SM on 148 SMs
 constexpr int DIAG_WIDTH = 7;                        // V, V*x, V*y, V*z, V*ux, V*uy, V*uz
 template <typename T> cudaError_t launch_sum_phi(cudaStream_t s, const T* C, size_t N, double* part);
 // launch_bubble_diag sums over the owned planes [g.zlo, g.zhi); zshift = global z of plane 0 (slabs).
-template <typename T> cudaError_t launch_bubble_diag(cudaStream_t s, const T* C, const T* U, Geom g, size_t N, int zshift, double* part);
+template <typename T> cudaError_t launch_bubble_diag(cudaStream_t s, const T* C, const T* U, Geom g, size_t N, int zshift, double ref, double* part);
 
 }  // namespace acm

@@ -11,14 +11,23 @@ namespace acm {
 // post-collision populations through store(ic, value).
 template <typename T, int Q, int COLL, typename Store>
 __device__ __forceinline__ void phase_collide(const T (&h)[Q], const Moments<Q, T, false>& m, T c0, T gx, T gy, T gz, T ux, T uy,
-                                              T uz, T one_minus_omega, T inv_xi, Store&& store)
+                                              T uz, T one_minus_omega, T inv_xi, T ref, Store&& store)
 {
-    const T phi = m.m0;
+    // fp32 instance (A22): h and phi are stored as deviations from the reference phase `ref` (0 or 1),
+    // h_i - ref w_i and phi - ref, so that the bulk of that phase keeps its digits; fp64: ref = 0, nothing changes
+    constexpr bool DEV = sizeof(T) == 4;
+    const T phid = m.m0;                             // stored zeroth moment
+    const T phi = DEV ? ref + phid : phid;           // the order parameter itself
     // interface normal (n = 0 where grad phi vanishes exactly) and theta = (1 - 4 (phi-1/2)^2)/xi
     const T g2 = gx * gx + gy * gy + gz * gz;
     const T inv = (g2 > T(0)) ? T(1) / sqrt(g2) : T(0);
-    const T dc = c0 - T(0.5);
-    const T theta = (T(1) - T(4) * dc * dc) * inv_xi;
+    T theta;
+    if constexpr (DEV) {
+        theta = T(4) * (ref + c0) * ((T(1) - ref) - c0) * inv_xi;     // 1 - 4 (phi - 1/2)^2 = 4 phi (1 - phi), c0 = phi_old - ref
+    } else {
+        const T dc = c0 - T(0.5);
+        theta = (T(1) - T(4) * dc * dc) * inv_xi;
+    }
     const T tnx = theta * inv * gx, tny = theta * inv * gy, tnz = theta * inv * gz;   // theta * n
 
     // closed form of the collision: h*_i = w_i [A + e_i.b + e_i e_i : T] (+ keep * h_i for SRT)
@@ -32,7 +41,8 @@ __device__ __forceinline__ void phase_collide(const T (&h)[Q], const Moments<Q, 
         const T dym = m.jy - phi * uy + sixth * tny;
         const T dzm = m.jz - phi * uz + sixth * tnz;
         const T p3 = T(3) * phi;
-        A = phi * (T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz));
+        const T usq = T(1.5) * (ux * ux + uy * uy + uz * uz);
+        A = DEV ? phid * (T(1) - usq) - ref * usq : phi * (T(1) - usq);        // DEV: phi (1 - usq) - ref
         bx = p3 * ux + T(0.5) * tnx + k * dxm;
         by = p3 * uy + T(0.5) * tny + k * dym;
         bz = p3 * uz + T(0.5) * tnz + k * dzm;
@@ -42,7 +52,9 @@ __device__ __forceinline__ void phase_collide(const T (&h)[Q], const Moments<Q, 
         // single relaxation time (A23): h*_i = (1-omega) h_i + omega phi Gamma_i(u) + (1-omega/2) F_i
         const T omega = T(1) - one_minus_omega;
         const T op = omega * phi, fh = T(1) - T(0.5) * omega;
-        A = op * (T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz));
+        const T usq = T(1.5) * (ux * ux + uy * uy + uz * uz);
+        // DEV: (1-omega) ref w_i + omega phi w_i (1 - usq) - ref w_i = w_i omega [phid (1 - usq) - ref usq]
+        A = DEV ? omega * (phid * (T(1) - usq) - ref * usq) : op * (T(1) - usq);
         bx = T(3) * op * ux + fh * tnx;
         by = T(3) * op * uy + fh * tny;
         bz = T(3) * op * uz + fh * tnz;
@@ -60,8 +72,9 @@ __device__ __forceinline__ void phase_collide(const T (&h)[Q], const Moments<Q, 
                                });
     } else {
         // fp32 instance (reading A22): the rest population is set by subtraction,
-        // h*_0 = phi_new - sum_{i>=1} h*_i, so that the collision conserves phi exactly in fp32.
-        T rest = phi;
+        // h*_0 = phi_new - sum_{i>=1} h*_i, so that the collision conserves phi exactly in fp32
+        // (all of them as deviations from ref w_i, which sum to ref).
+        T rest = phid;
         emit_populations<Q, T>(A, bx, by, bz, Ts * ux * ux, Ts * uy * uy, Ts * uz * uz, Ts * ux * uy, Ts * ux * uz,
                                Ts * uy * uz, [&](auto ic, T v) {
                                    constexpr int i = decltype(ic)::value;
@@ -93,11 +106,13 @@ __device__ __forceinline__ HydroCell<T> hydro_velocity(const Moments<Q, T, true>
     const T pstar = m.m0;
     const T p3 = pstar * T(1.0 / 3.0);
 
+    // fp32 instance: c0 = phi - ref (see phase_collide); a.rho_L and a.tau_L then hold the values AT phi = ref
     const T rho = a.rho_L + c0 * a.drho;                  // eq. 8 (phi_L = 0)
     const T inv_rho = T(1) / rho;
     const T tau = a.tau_L + c0 * a.dtau;                  // eq. 20
     const T s_nu = T(1) / (tau + T(0.5));                 // eq. 21
-    const T mu = a.beta4 * c0 * (c0 - T(1)) * (c0 - T(0.5)) - a.kappa * lap;   // eq. 17
+    const T mu = (sizeof(T) == 4 ? a.beta4 * (a.ref + c0) * (c0 - (T(1) - a.ref)) * (c0 + (a.ref - T(0.5)))
+                                 : a.beta4 * c0 * (c0 - T(1)) * (c0 - T(0.5))) - a.kappa * lap;   // eq. 17
     const T grx = a.drho * gpx, gry = a.drho * gpy, grz = a.drho * gpz;
 
     // deviatoric second moment without the velocity part

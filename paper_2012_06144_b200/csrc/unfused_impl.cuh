@@ -64,7 +64,7 @@ __global__ void __launch_bounds__(ACM_MAXT) collide_h_kernel(const PhaseArgs<T> 
     Moments<Q, T, false> m;
     m.compute(h);
     m.m0 = a.Cdst[idx];          // the phase field written by phi_kernel
-    phase_collide<T, Q, COLL>(h, m, c0, gx, gy, gz, ux, uy, uz, a.one_minus_omega, a.inv_xi, [&](auto ic, T v) {
+    phase_collide<T, Q, COLL>(h, m, c0, gx, gy, gz, ux, uy, uz, a.one_minus_omega, a.inv_xi, a.ref, [&](auto ic, T v) {
         st_stream(a.Hdst + (size_t) decltype(ic)::value * N + idx, v);
     });
 }

@@ -40,8 +40,12 @@ def test_fp32_one_step(Qh, Qg, walls):
     a.step(1)
     ho, go = o.get_pdfs()
     ha, ga = a.get_pdfs()
-    assert np.abs(ha.cpu().numpy() - ho).max() < 2e-7
-    assert np.abs(ga.cpu().numpy() - go).max() < 2e-7
+    dh = np.abs(ha.cpu().numpy() - ho)
+    assert dh[1:].max() < 5e-8                 # a few ulp of 0.07
+    # rest population by subtraction (A22): Q-1 roundings of ulp(0.07)/2 = 3.7e-9 each, the same again in phi = sum h,
+    # and the un-shifting h' + ref w_0 (ulp(0.3)/2 = 1.5e-8)
+    assert dh[0].max() < 4e-7
+    assert np.abs(ga.cpu().numpy() - go).max() < 2e-8
     po, uo, _ = o.fields(False)
     pa, ua, _ = a.fields(False)
     assert np.abs(pa.cpu().numpy() - po).max() < 5e-7
