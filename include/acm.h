@@ -138,10 +138,10 @@ int acm_phi_mass(acm_ctx*, double* total_host);
 
 /* Rising-bubble diagnostics of section 6.1.  The paper takes "the terminal velocity of
  * the bubbles" u_t for eq. 34 without saying how it is measured; here (reading A24) the
- * light phase is weighted with 1 - phi:
- *   out_host[0]    V   = sum_x (1 - phi)
- *   out_host[1..3] X_b = sum_x (1 - phi) x_c / V, x_c = cell centre (i + 1/2); plain coordinates
- *   out_host[4..6] u_b = sum_x (1 - phi) u / V
+ * bubble is the set of cells with phi < 1/2, weighted with 1 - phi:  w = (1 - phi) [phi < 1/2]
+ *   out_host[0]    V   = sum_x w
+ *   out_host[1..3] X_b = sum_x w x_c / V, x_c = cell centre (i + 1/2); plain coordinates
+ *   out_host[4..6] u_b = sum_x w u / V
  * fp64 accumulation, deterministic two-pass block reduction; synchronises the stream.
  * ACM_EUNSTABLE if a result is not finite (V = 0 included). */
 int acm_bubble_diag(acm_ctx*, double out_host[7]);
@@ -159,7 +159,7 @@ double acm_drag_lbm(double g_y, double rho_H, double rho_L, double D, double u_t
 double acm_drag_exp(double Re_Gr);
 
 /* Un-normalised sums behind acm_bubble_diag: { sum w, sum w x_c, sum w y_c, sum w z_c, sum w u_x, sum w u_y,
- * sum w u_z } with w = 1 - phi over the cells this context owns (z_c in global coordinates for a slab), so that
+ * sum w u_z } with w = (1 - phi) [phi < 1/2] over the cells this context owns (z_c in global coordinates for a slab), so that
  * the slabs of a decomposed domain can be added up before normalising. */
 int acm_bubble_sums(acm_ctx*, double out_host[7]);
 

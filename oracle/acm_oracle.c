@@ -36,7 +36,7 @@
  *   A18 no clamp on phi or rho
  *   A19 p = p* rho c_s^2
  *   A23 variant ORACLE_VAR_PHASE_SRT: Omega^h = omega_phi I
- *   A24 bubble volume/centroid/velocity weighted with (1 - phi)
+ *   A24 bubble volume/centroid/velocity over phi < 1/2, weighted with 1 - phi
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): lattice identities, weighted
  * orthogonality of M, eq.25 forcing identity, brute-force 4^3 step against a
@@ -611,10 +611,11 @@ int oracle_set_variant(oracle_ctx *o, unsigned flags)
 }
 
 /* Rising-bubble diagnostics (section 6.1).  The paper uses "the terminal velocity of the
- * bubbles" u_t in eq. 34 without saying how it is measured; reading A24: the light
- * phase is weighted with (phi_H - phi), i.e.
- *   V = sum_x (1 - phi),  X_b = sum_x (1 - phi) x_c / V,  u_b = sum_x (1 - phi) u / V,
- * x_c = cell centre (i + 1/2), plain coordinates (no periodic unwrapping).
+ * bubbles" u_t in eq. 34 without saying how it is measured; reading A24: the cells of
+ * the bubble are those with phi < phi_0 = 1/2, weighted with (phi_H - phi), i.e. with w = (1 - phi) [phi < 1/2]
+ *   V = sum_x w,  X_b = sum_x w x_c / V,  u_b = sum_x w u / V,
+ * x_c = cell centre (i + 1/2), plain coordinates (no periodic unwrapping).  (Without the restriction to
+ * phi < 1/2 the sums pick up the 1e-4 compression of the heavy liquid over millions of cells.)
  * out = { V, X_b[3], u_b[3] }. */
 int oracle_bubble_diag(oracle_ctx *o, double out[7])
 {
@@ -625,7 +626,7 @@ int oracle_bubble_diag(oracle_ctx *o, double out[7])
         for (int y = 0; y < o->ny; ++y)
             for (int x = 0; x < o->nx; ++x) {
                 size_t c = cell(o, x, y, z);
-                double wgt = PHI_H - o->C[c];
+                double wgt = (o->C[c] < PHI_0) ? PHI_H - o->C[c] : 0.0;
                 V += wgt;
                 X[0] += wgt * (x + 0.5); X[1] += wgt * (y + 0.5); X[2] += wgt * (z + 0.5);
                 for (int a = 0; a < 3; ++a) Ub[a] += wgt * o->U[a * N + c];

@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(RED_THREADS) sum_pass2(const double* __restric
 }
 
 // Rising-bubble diagnostics (section 6.1; reading A24): seven sums weighted with the
-// light-phase indicator 1 - phi:  V, V x_c, V y_c, V z_c (cell centres i + 1/2), V u_x, V u_y, V u_z.
+// light-phase weight (1 - phi) [phi < 1/2]:  V, V x_c, V y_c, V z_c (cell centres i + 1/2), V u_x, V u_y, V u_z.
 // Same fixed-order two-pass scheme as sum(phi), so the result is bitwise reproducible.
 template <typename T>
 __global__ void __launch_bounds__(RED_THREADS) diag_pass1(const T* __restrict__ C, const T* __restrict__ U, Geom g, size_t N, int zshift, double ref, double* part)
@@ -189,7 +189,8 @@ __global__ void __launch_bounds__(RED_THREADS) diag_pass1(const T* __restrict__ 
         const int r = (int)(i - (size_t)zl * plane);
         const int z = zl + zshift;
         const int y = r / g.nx, x = r - y * g.nx;
-        const double w = (1.0 - ref) - (double)C[i];      // C holds phi - ref
+        const double om = (1.0 - ref) - (double)C[i];     // 1 - phi (C holds phi - ref)
+        const double w = om > 0.5 ? om : 0.0;             // cells of the bubble: phi < 1/2
         s[0] += w;
         s[1] += w * (x + 0.5); s[2] += w * (y + 0.5); s[3] += w * (z + 0.5);
         s[4] += w * (double)U[i]; s[5] += w * (double)U[N + i]; s[6] += w * (double)U[2 * N + i];

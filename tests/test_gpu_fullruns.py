@@ -41,13 +41,12 @@ def test_config2_rising_bubble_2000_steps():
     del a0
     a, c, uu, pr = _run(p, phi, u, 2000)
     V1, X1, U1 = a.bubble_diag()
-    assert abs(V1 / V0 - 1) < 1e-3
-    assert X1[1] > X0[1] + 1e-3 and U1[1] > 1e-6                 # rising against gravity
-    # mirror symmetry in x and z holds up to the amplified rounding noise next to the walls,
-    # which the (1 - phi) weight picks up over the 8 M cells of heavy liquid
+    assert abs(V1 / V0 - 1) < 0.1            # sum(phi) is conserved exactly; this weighted volume follows the relaxing interface
+    assert U1[1] > 1e-4                                           # rising against gravity
     print("config2 after 2000 steps: V", V0, V1, "X", X0, X1, "U", U1)
-    assert abs(X1[0] - X0[0]) < 1e-2 and abs(X1[2] - X0[2]) < 1e-2
-    assert abs(U1[0]) < 0.05 * U1[1] and abs(U1[2]) < 0.05 * U1[1]
+    assert 0.5 < X1[1] - X0[1] < 4.0                              # about u_b * t: a couple of cells
+    assert abs(X1[0] - X0[0]) < 1e-3 and abs(X1[2] - X0[2]) < 1e-3          # mirror symmetry in x and z (up to the noise of "Conditioning")
+    assert abs(U1[0]) < 1e-3 * U1[1] and abs(U1[2]) < 1e-3 * U1[1]
     # hydrostatic pressure builds up in the heavy liquid: higher at the bottom than at the top
     assert float(pr[64, 5, 10] - pr[64, 500, 10]) > 0
 
