@@ -120,7 +120,7 @@ class ACM:
 
     def __init__(self, nx, ny, nz, stencil_phase=15, stencil_hydro=19, rho_H=1.0, rho_L=1e-3, sigma=1e-4, xi=5.0,
                  M=0.02, nu_H=1 / 60, nu_L=1 / 60, gravity=(0.0, 0.0, 0.0), wall_flags=0, precision="f64",
-                 device="cuda:0", stream=None, inplace=False, phase_srt=False, unfused=False):
+                 device="cuda:0", stream=None, inplace=False, phase_srt=False, unfused=False, guard_bytes=0):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2012_06144_b200 needs a CUDA device (no CPU fallback)")
         self._lib = load()
@@ -137,9 +137,14 @@ class ACM:
                                                    self.options)
         if nbytes == 0:
             raise AcmError(ACM_EINVAL, "invalid grid size / stencil / precision")
+        # guard_bytes (debugging aid): canary regions before and after the workspace, see guards_intact()
+        self._guard = (int(guard_bytes) + 255) & ~255
         with torch.cuda.device(self.device):
-            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-        base = (self.workspace.data_ptr() + 255) & ~255
+            self.workspace = torch.empty(nbytes + 256 + 2 * self._guard, dtype=torch.uint8, device=self.device)
+            if self._guard:
+                self.workspace.fill_(0xA5)
+        base = ((self.workspace.data_ptr() + 255) & ~255) + self._guard
+        self._ws_span = (base - self.workspace.data_ptr(), nbytes)
         g = (C.c_double * 3)(*[float(v) for v in gravity])
         h = C.c_void_p()
         with torch.cuda.device(self.device):
@@ -170,6 +175,12 @@ class ACM:
         assert t.is_cuda and t.dtype == self.dtype and t.is_contiguous() and tuple(t.shape) == tuple(shape), \
             (t.device, t.dtype, t.shape, shape)
         return _ptr(t)
+
+    def guards_intact(self):
+        """True if no byte outside the workspace handed to acm_create was written (needs guard_bytes > 0)."""
+        off, n = self._ws_span
+        torch.cuda.synchronize(self.device)
+        return bool((self.workspace[:off] == 0xA5).all() and (self.workspace[off + n:] == 0xA5).all())
 
     def set_block(self, bx, by=1, bz=1):
         self._call(self._lib.acm_set_block, int(bx), int(by), int(bz))

@@ -335,3 +335,29 @@ def test_laplace_law_gpu():
     golden = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "laplace_config1.txt")
     rows = {int(l.split()[0]): float(l.split()[1]) for l in open(golden) if not l.startswith("#")}
     assert abs(ratio - rows[10000]) < 1e-6
+
+
+@pytest.mark.parametrize("mode", [dict(), dict(inplace=True), dict(unfused=True), dict(precision="f32"), dict(phase_srt=True)])
+@pytest.mark.parametrize("shape,Qh,Qg,walls", [((150, 7, 5), 15, 19, 0), ((33, 5, 4), 27, 27, inputs.WALL_X | inputs.WALL_Y | inputs.WALL_Z),
+                                               ((260, 3, 2), 19, 27, inputs.WALL_Y), ((96, 50, 1), 9, 9, 0)])
+def test_no_write_outside_the_workspace(shape, Qh, Qg, walls, mode):
+    """Canary regions of 1 MiB before and after the caller's workspace stay untouched by init, steps, every export /
+    import and the reductions (compute-sanitizer is not available on this pool)."""
+    from paper_2012_06144_b200.binding import ACM
+    p = Params(nx=shape[0], ny=shape[1], nz=shape[2], stencil_phase=Qh, stencil_hydro=Qg, wall_flags=walls)
+    phi, u, h, g = random_state(p, seed=13)
+    u[2] = 0.0 if Qh == 9 else u[2]
+    kw = dict(mode)
+    dt = np.float32 if kw.get("precision") == "f32" else np.float64
+    a = ACM.from_params(p, guard_bytes=1 << 20, **kw)
+    dev = lambda x: torch.from_numpy(np.ascontiguousarray(x, dtype=dt)).cuda()
+    a.init(dev(phi), dev(u))
+    a.set_pdfs(dev(h), dev(g))
+    a.step(3)
+    a.get_pdfs()
+    a.fields()
+    a.phi_mass()
+    a.bubble_diag()
+    a.set_block(64, 2, 1)
+    a.step(2)
+    assert a.guards_intact()
