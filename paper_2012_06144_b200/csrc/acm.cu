@@ -166,7 +166,7 @@ static int launch_phase_range(acm_ctx* c, int z0, int z1)
     a.Csrc = wsp<T>(c, c->offC[c->curC]); a.Cdst = wsp<T>(c, c->offC[c->curC ^ 1]);
     a.U = wsp<T>(c, c->offU[c->curU]);
     a.g = geom_of(c, lb_linear(c), z0, z1);
-    a.N = c->N;
+    a.N = (unsigned)c->N;
     const double omega = 1.0 / (3.0 * c->M + 0.5);     // tau_phi = M/c_s^2 (eq. 2), shifted by 1/2
     a.one_minus_omega = (T)(1.0 - omega);
     a.inv_xi = (T)(1.0 / c->xi);
@@ -194,7 +194,7 @@ static int launch_hydro_range(acm_ctx* c, int z0, int z1)
     a.C = wsp<T>(c, c->offC[c->curC]);
     a.U = wsp<T>(c, c->offU[c->curU]);
     a.g = geom_of(c, lb_linear(c), z0, z1);
-    a.N = c->N;
+    a.N = (unsigned)c->N;
     // rho and tau at the reference phase of the stored phi (ref = 0: the light phase, as in eqs. 8, 20)
     a.ref = (T)c->ref;
     a.rho_L = (T)(c->rho_L + c->ref * (c->rho_H - c->rho_L)); a.drho = (T)(c->rho_H - c->rho_L);
@@ -363,7 +363,9 @@ static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase,
     c->stH = c->stG = ST_POST;
     c->initialised = false;
     c->sticky = ACM_OK;
-    c->block = dim3(128, 1, 1);
+    // one block = 1 KB of every population row (measured best on B200 for both precisions, profiles/): 128 fp64
+    // or 256 fp32 cells along x; fp32 falls back to 128 when nx is not a multiple of 256
+    c->block = (precision == ACM_F32 && nx % 256 == 0) ? dim3(256, 1, 1) : dim3(128, 1, 1);
     c->launches = 0;
     c->profiling = false;
     *out = c;

@@ -35,7 +35,7 @@ __global__ void init_kernel(const T* __restrict__ phi, const T* __restrict__ u, 
     if (!cell_of_thread(g, x, y, z)) return;
     Nbr nb;
     nb.setup<true>(g, x, y, z);
-    const int idx = nb.at<0, 0, 0>();
+    const unsigned idx = nb.at<0, 0, 0>();
     const T ph = phi[idx];
     const T ux = u[idx], uy = u[N + idx], uz = u[2 * N + idx];
     C[idx] = ph - ref;
@@ -61,7 +61,7 @@ __global__ void init_kernel(const T* __restrict__ phi, const T* __restrict__ u, 
             constexpr int o = L::opp(i);
             v = gamma_i<QG, T>(L::ex(o), L::ey(o), L::ez(o), T(L::w(o)), ux, uy, uz) - T(L::w(o));
         } else {
-            const int j = nb.template at<ex, ey, ez>();
+            const unsigned j = nb.template at<ex, ey, ez>();
             v = gamma_i<QG, T>(ex, ey, ez, T(L::w(i)), u[j], u[N + j], u[2 * N + j]) - T(L::w(i));
         }
         G[(size_t)i * N + idx] = v;
@@ -80,7 +80,7 @@ __global__ void export_kernel(const T* F, const T* __restrict__ C, T* out, T* p,
     if (!cell_of_thread(g, x, y, z)) return;
     Nbr nb;
     nb.setup<true>(g, x, y, z);
-    const int idx = nb.at<0, 0, 0>();
+    const unsigned idx = nb.at<0, 0, 0>();
     T f[Q];
     if constexpr (POST) static_for<0, Q>([&](auto ic) { constexpr int i = decltype(ic)::value; f[i] = load_post<Q, i, T, STATE>(F, N, nb); });
     else load_incoming<Q, T, true, STATE>(F, N, nb, f);
@@ -106,7 +106,7 @@ __global__ void import_kernel(const T* __restrict__ in, T* F, Geom g, size_t N, 
     if (!cell_of_thread(g, x, y, z)) return;
     Nbr nb;
     nb.setup<true>(g, x, y, z);
-    const int idx = nb.at<0, 0, 0>();
+    const unsigned idx = nb.at<0, 0, 0>();
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
         using L = Lat<Q>;

@@ -51,8 +51,9 @@ __device__ __forceinline__ bool cell_of_thread(const Geom& g, int& x, int& y, in
 // Per-cell neighbourhood: coordinates of x-1, x, x+1 (periodic wrap; clamped at a wall, which is
 // the mirror ghost phi(x,-1,z) = phi(x,0,z) of the FD stencils) and "beyond a wall" flags.
 struct Nbr {
-    int xs[3];        // x-1, x, x+1
-    int row[3][3];    // [dz+1][dy+1] -> (z'*ny + y')*nx
+    // unsigned: cell indices are < 2^31 and a zero-extended index costs one wide multiply-add per address
+    unsigned xs[3];        // x-1, x, x+1
+    unsigned row[3][3];    // [dz+1][dy+1] -> (z'*ny + y')*nx
     bool wxm, wxp, wym, wyp, wzm, wzp;   // the cell at x-1 / x+1 / ... lies beyond a wall
 
     template <bool WALLS>
@@ -67,16 +68,16 @@ struct Nbr {
         // z: wall -> clamp; ghost planes -> use them as they are; else periodic wrap inside [zlo, zhi)
         if (zm < g.zlo) { if (WALLS && (g.walls & WALL_ZLO)) { wzm = true; zm = g.zlo; } else if (!g.zghost) zm = g.zhi - 1; }
         if (zp >= g.zhi) { if (WALLS && (g.walls & WALL_ZHI)) { wzp = true; zp = g.zhi - 1; } else if (!g.zghost) zp = g.zlo; }
-        xs[0] = xm; xs[1] = x; xs[2] = xp;
+        xs[0] = (unsigned)xm; xs[1] = (unsigned)x; xs[2] = (unsigned)xp;
         const int ys[3] = {ym, y, yp}, zs[3] = {zm, z, zp};
 #pragma unroll
         for (int a = 0; a < 3; ++a)
 #pragma unroll
-            for (int b = 0; b < 3; ++b) row[a][b] = (zs[a] * g.ny + ys[b]) * g.nx;
+            for (int b = 0; b < 3; ++b) row[a][b] = (unsigned)((zs[a] * g.ny + ys[b]) * g.nx);
     }
     // index of the cell at offset (dx,dy,dz), each in {-1,0,1}
     template <int DX, int DY, int DZ>
-    __device__ __forceinline__ int at() const { return row[DZ + 1][DY + 1] + xs[DX + 1]; }
+    __device__ __forceinline__ unsigned at() const { return row[DZ + 1][DY + 1] + xs[DX + 1]; }
     // is the cell at offset (dx,dy,dz) beyond a wall?
     template <int DX, int DY, int DZ, bool WALLS>
     __device__ __forceinline__ bool beyond() const
@@ -246,7 +247,7 @@ struct PhaseArgs {
     const T* Csrc; T* Cdst;
     const T* U;
     Geom g;
-    size_t N;
+    unsigned N;      // cells per population plane (< 2^31): 32 bits keep the plane offsets i*N one wide multiply
     T one_minus_omega, inv_xi;
     T ref;           // fp32 instance: reference phase of the deviation storage (0 or 1); 0 for fp64
 };
@@ -257,7 +258,7 @@ struct HydroArgs {
     const T* C;      // new phi
     T* U;
     Geom g;
-    size_t N;
+    unsigned N;      // cells per population plane (< 2^31): 32 bits keep the plane offsets i*N one wide multiply
     T rho_L, drho, tau_L, dtau, beta4, kappa, gx, gy, gz;
     T ref;           // as in PhaseArgs; rho_L, tau_L are the values at phi = ref
 };

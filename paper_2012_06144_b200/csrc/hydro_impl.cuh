@@ -20,8 +20,8 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const H
     if (!cell_of_thread(a.g, x, y, z)) return;
     Nbr nb;
     nb.setup<WALLS>(a.g, x, y, z);
-    const int idx = nb.at<0, 0, 0>();
-    const size_t N = a.N;
+    const unsigned idx = nb.at<0, 0, 0>();
+    const size_t N = a.N;      // zero-extended 32-bit value
 
     T g[Q];
     load_incoming<Q, T, WALLS, STATE>(a.Gsrc, N, nb, g);

@@ -18,8 +18,8 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const P
     if (!cell_of_thread(a.g, x, y, z)) return;
     Nbr nb;
     nb.setup<WALLS>(a.g, x, y, z);
-    const int idx = nb.at<0, 0, 0>();
-    const size_t N = a.N;
+    const unsigned idx = nb.at<0, 0, 0>();
+    const size_t N = a.N;      // zero-extended 32-bit value
 
     T h[Q];
     load_incoming<Q, T, WALLS, STATE>(a.Hsrc, N, nb, h);

@@ -24,7 +24,7 @@ __global__ void __launch_bounds__(ACM_MAXT) stream_kernel(const T* __restrict__ 
     if (!cell_of_thread(g, x, y, z)) return;
     Nbr nb;
     nb.setup<WALLS>(g, x, y, z);
-    const int idx = nb.at<0, 0, 0>();
+    const unsigned idx = nb.at<0, 0, 0>();
     T f[Q];
     load_incoming<Q, T, WALLS, ST_POST>(src, N, nb, f);
     static_for<0, Q>([&](auto ic) { constexpr int i = decltype(ic)::value; st_stream(dst + (size_t)i * N + idx, f[i]); });
@@ -53,8 +53,8 @@ __global__ void __launch_bounds__(ACM_MAXT) collide_h_kernel(const PhaseArgs<T> 
     if (!cell_of_thread(a.g, x, y, z)) return;
     Nbr nb;
     nb.setup<WALLS>(a.g, x, y, z);
-    const int idx = nb.at<0, 0, 0>();
-    const size_t N = a.N;
+    const unsigned idx = nb.at<0, 0, 0>();
+    const size_t N = a.N;      // zero-extended 32-bit value
     T h[Q];
     static_for<0, Q>([&](auto ic) { constexpr int i = decltype(ic)::value; h[i] = ld_stream(a.Hdst + (size_t)i * N + idx); });
     const T ux = __ldg(a.U + idx), uy = __ldg(a.U + N + idx), uz = __ldg(a.U + 2 * N + idx);
@@ -78,8 +78,8 @@ __global__ void __launch_bounds__(ACM_MAXT) velocity_kernel(const HydroArgs<T> a
     if (!cell_of_thread(a.g, x, y, z)) return;
     Nbr nb;
     nb.setup<WALLS>(a.g, x, y, z);
-    const int idx = nb.at<0, 0, 0>();
-    const size_t N = a.N;
+    const unsigned idx = nb.at<0, 0, 0>();
+    const size_t N = a.N;      // zero-extended 32-bit value
     T g[Q];
     static_for<0, Q>([&](auto ic) { constexpr int i = decltype(ic)::value; g[i] = ld_stream(a.Gdst + (size_t)i * N + idx); });
     const T uox = Uold[idx], uoy = Uold[N + idx], uoz = Uold[2 * N + idx];
@@ -101,8 +101,8 @@ __global__ void __launch_bounds__(ACM_MAXT) collide_g_kernel(const HydroArgs<T> 
     if (!cell_of_thread(a.g, x, y, z)) return;
     Nbr nb;
     nb.setup<WALLS>(a.g, x, y, z);
-    const int idx = nb.at<0, 0, 0>();
-    const size_t N = a.N;
+    const unsigned idx = nb.at<0, 0, 0>();
+    const size_t N = a.N;      // zero-extended 32-bit value
     T g[Q];
     static_for<0, Q>([&](auto ic) { constexpr int i = decltype(ic)::value; g[i] = ld_stream(a.Gdst + (size_t)i * N + idx); });
     const T uox = Uold[idx], uoy = Uold[N + idx], uoz = Uold[2 * N + idx];
