@@ -210,16 +210,16 @@ __device__ __forceinline__ T load_post(const T* F, size_t N, const Nbr& nb)
 // Isotropic finite differences of phi on lattice Q (eqs. 23, 24 with c = dx = 1, c_s^2 = 1/3):
 //   grad phi = 3 sum_i w_i e_i phi(x+e_i)      (summed as opposite-pair differences)
 //   lap  phi = 6 sum_i w_i [phi(x+e_i) - phi(x)]
-template <int Q, typename T, bool LAPLACE>
-__device__ __forceinline__ void fd_phi(const T* __restrict__ C, const Nbr& nb, T c0, T& gx, T& gy, T& gz, T& lap)
+template <int Q, typename T, bool LAPLACE, typename Acc>
+__device__ __forceinline__ void fd_phi_acc(const Acc& acc, T c0, T& gx, T& gy, T& gz, T& lap)
 {
     using L = Lat<Q>;
     T dx[4] = {0, 0, 0, 0}, dy[4] = {0, 0, 0, 0}, dz[4] = {0, 0, 0, 0}, ss[4] = {0, 0, 0, 0};   // per class
     static_for<1, Q, 2>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
         constexpr int ex = L::ex(i), ey = L::ey(i), ez = L::ez(i), c = L::cls(i);
-        const T p = __ldg(C + nb.template at<ex, ey, ez>());
-        const T m = __ldg(C + nb.template at<-ex, -ey, -ez>());
+        const T p = acc.template get<ex, ey, ez>();
+        const T m = acc.template get<-ex, -ey, -ez>();
         const T d = p - m;
         addsgn<ex>(dx[c], d); addsgn<ey>(dy[c], d); addsgn<ez>(dz[c], d);
         if constexpr (LAPLACE) ss[c] += p + m;
@@ -237,6 +237,46 @@ __device__ __forceinline__ void fd_phi(const T* __restrict__ C, const Nbr& nb, T
     (void)wsum;
     if constexpr (LAPLACE) lap = l - T(6.0 * (1.0 - L::wc(0))) * c0;   // sum_{i>=1} w_i = 1 - w_0
 }
+
+// where the phi stencil reads from: global memory through L1/L2 (default), or a shared-memory tile of the
+// block's 3 x 3 neighbouring rows (the ACM_PHI_SMEM experiment, profiles/r1b_profiles.md)
+template <typename T>
+struct PhiGlobal {
+    const T* C;
+    const Nbr* nb;
+    template <int DX, int DY, int DZ> __device__ __forceinline__ T get() const { return __ldg(C + nb->template at<DX, DY, DZ>()); }
+};
+template <typename T>
+struct PhiTile {
+    const T* tile;     // [3][3][W]
+    int W, tx;
+    template <int DX, int DY, int DZ> __device__ __forceinline__ T get() const { return tile[((DZ + 1) * 3 + (DY + 1)) * W + tx + 1 + DX]; }
+};
+
+template <int Q, typename T, bool LAPLACE>
+__device__ __forceinline__ void fd_phi(const T* __restrict__ C, const Nbr& nb, T c0, T& gx, T& gy, T& gz, T& lap)
+{
+    fd_phi_acc<Q, T, LAPLACE>(PhiGlobal<T>{C, &nb}, c0, gx, gy, gz, lap);
+}
+
+#ifdef ACM_PHI_SMEM
+// Cooperative load of the 9 rows (dy, dz in -1..1) of phi around the block's x-row, plus one halo cell on each
+// side, into shared memory.  Valid for 3-D launches with blocks of shape (bx, 1, 1): y and z are uniform per block.
+template <typename T>
+__device__ __forceinline__ void load_phi_tile(T* tile, const T* __restrict__ C, const Nbr& nb, int W, bool last_in_row)
+{
+    const int tx = threadIdx.x;
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            T* row = tile + (a * 3 + b) * W;
+            row[tx + 1] = __ldg(C + nb.row[a][b] + nb.xs[1]);
+            if (tx == 0) row[0] = __ldg(C + nb.row[a][b] + nb.xs[0]);
+            if (last_in_row) row[tx + 2] = __ldg(C + nb.row[a][b] + nb.xs[2]);
+        }
+}
+#endif
 
 // ------------------------------------------------------------------------------------------
 // argument blocks of the two LB kernels

@@ -17,9 +17,22 @@ template <typename T, int Q, bool WALLS, int STATE>
 __global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const HydroArgs<T> a)
 {
     int x, y, z;
+#ifdef ACM_PHI_SMEM
+    __shared__ T phi_tile[9 * (ACM_MAXT + 2)];
+    const bool active = cell_of_thread(a.g, x, y, z);
+    const bool tiled = !a.g.linear && blockDim.y == 1 && blockDim.z == 1;      // uniform over the block
+    Nbr nb;
+    if (active) nb.setup<WALLS>(a.g, x, y, z);
+    if (tiled) {
+        if (active) load_phi_tile<T>(phi_tile, a.C, nb, (int)blockDim.x + 2, threadIdx.x == blockDim.x - 1 || x == a.g.nx - 1);
+        __syncthreads();
+    }
+    if (!active) return;
+#else
     if (!cell_of_thread(a.g, x, y, z)) return;
     Nbr nb;
     nb.setup<WALLS>(a.g, x, y, z);
+#endif
     const unsigned idx = nb.at<0, 0, 0>();
     const size_t N = a.N;      // zero-extended 32-bit value
 
@@ -28,6 +41,10 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const H
     const T uox = a.U[idx], uoy = a.U[N + idx], uoz = a.U[2 * N + idx];
     const T c0 = __ldg(a.C + idx);
     T gpx, gpy, gpz, lap;
+#ifdef ACM_PHI_SMEM
+    if (tiled) fd_phi_acc<Q, T, true>(PhiTile<T>{phi_tile, (int)blockDim.x + 2, (int)threadIdx.x}, c0, gpx, gpy, gpz, lap);
+    else
+#endif
     fd_phi<Q, T, true>(a.C, nb, c0, gpx, gpy, gpz, lap);
 
     Moments<Q, T, true> m;
