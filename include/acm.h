@@ -210,6 +210,18 @@ int acm_slab_info(const acm_ctx*, int info[6]);
 enum { ACM_HALO_H = 0, ACM_HALO_G = 1, ACM_HALO_PHI = 2 };
 int acm_halo_plan(const acm_ctx*, int what, int side, int recv, int max_chunks, size_t* offsets, size_t* bytes);
 
+/* Peer mode of a slab: instead of reading ghost planes that an exchange has filled, the two LB kernels read the
+ * planes just outside the owned range straight from the NEIGHBOUR slabs' workspaces -- the populations they pull
+ * across the face and the phi stencil -- so that no population or phi plane is copied at all and the only thing
+ * the ranks exchange per kernel is a completion signal.  lo_workspace / hi_workspace: [device] base pointers of the
+ * workspaces the low-z / high-z neighbour contexts were created on, valid on this device: another context of the
+ * same process, a CUDA-IPC mapping of another process's allocation, or a peer GPU's memory with peer access
+ * enabled (NVLink).  The neighbour of the outermost slab of a periodic domain is the slab at the other end; a face
+ * on a z wall needs no pointer (NULL).  All slabs must have the same height (nz_global % nranks == 0) and advance in
+ * lockstep: the caller guarantees that a neighbour has finished kernel n-1 before this slab launches kernel n.
+ * Both NULL switches peer mode off.  acm_get_pdfs / acm_fields(p) still read ghost planes: refresh them first. */
+int acm_set_peers(acm_ctx*, void* lo_workspace, void* hi_workspace);
+
 /* Launch one LB kernel on the owned planes [z0, z1) (0 <= z0 <= z1 <= owned planes; empty range = no launch)
  * without flipping the buffers; the *_commit call flips them once all planes of the step are launched.
  * Also valid on a plain context, where acm_step(1) equals launch(0, nz), commit for both kernels. */

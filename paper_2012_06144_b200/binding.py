@@ -19,7 +19,7 @@ ACM_OPT_INPLACE, ACM_OPT_PHASE_SRT, ACM_OPT_UNFUSED = 1, 2, 4
 
 EXPORTS = ["acm_workspace_bytes", "acm_workspace_bytes_opt", "acm_create", "acm_create_opt", "acm_init", "acm_step", "acm_fields", "acm_phi_mass", "acm_get_pdfs",
            "acm_set_pdfs", "acm_run_host", "acm_set_reference_phase", "acm_bubble_diag", "acm_bubble_sums", "acm_slab_range", "acm_workspace_bytes_slab", "acm_create_slab", "acm_slab_info",
-           "acm_halo_plan", "acm_phase_launch", "acm_phase_commit", "acm_hydro_launch", "acm_hydro_commit", "acm_bubble_params", "acm_drag_lbm", "acm_drag_exp", "acm_set_block", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
+           "acm_halo_plan", "acm_set_peers", "acm_phase_launch", "acm_phase_commit", "acm_hydro_launch", "acm_hydro_commit", "acm_bubble_params", "acm_drag_lbm", "acm_drag_exp", "acm_set_block", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
 
 _lib = None
 
@@ -69,6 +69,7 @@ def load(build_if_missing: bool = True):
     lib.acm_create_slab.argtypes = [C.POINTER(vp)] + [i32] * 5 + [dbl] * 7 + [C.POINTER(dbl), C.c_uint, i32, C.c_uint, i32, i32, vp, vp]
     lib.acm_slab_info.argtypes = [vp, C.POINTER(i32)]
     lib.acm_halo_plan.argtypes = [vp, i32, i32, i32, i32, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
+    lib.acm_set_peers.argtypes = [vp, vp, vp]
     lib.acm_phase_launch.argtypes = [vp, i32, i32]
     lib.acm_phase_commit.argtypes = [vp]
     lib.acm_hydro_launch.argtypes = [vp, i32, i32]

@@ -41,6 +41,9 @@ struct acm_ctx {
     // slab of a z-decomposed domain (acm_create_slab); a plain context owns everything: nzl = nz, zlo = 0
     int nzl, zlo, ghost;                  // owned planes [zlo, zlo+nzl), ghost = 1: planes zlo-1 and zlo+nzl are halos
     int zglob0, nz_global, rank, nranks;  // global z of the first owned plane, global height, position in the decomposition
+    // peer mode of a slab (acm_set_peers): workspaces of the neighbour slabs, read directly by the LB kernels
+    bool peer_on;
+    char *peer_lo, *peer_hi;
     // fp32 instance: h and phi are stored as deviations from the reference phase (A22)
     int ref_mode;                         // -1: chosen by acm_init (the majority phase; heavy for slabs), else 0 / 1
     double ref;                           // 0 or 1; always 0 for fp64
@@ -155,6 +158,16 @@ static int init_t(acm_ctx* c, const void* phi, const void* u)
 // state of the array after a step that read it in state s
 static int next_state(int s) { return s == ST_POST ? ST_POST : (s == ST_IN ? ST_SWAP : ST_IN); }
 
+// Peer mode: the neighbours' array at the same workspace offset, shifted by the slab height so that this slab's
+// index of the plane just below (above) its owned range addresses the neighbour's last (first) owned plane.
+template <typename T>
+static Peers<T> peers_at(const acm_ctx* c, size_t off)
+{
+    if (!c->peer_on) return Peers<T>{nullptr, nullptr};
+    const ptrdiff_t shift = (ptrdiff_t)c->nzl * c->nx * c->ny;
+    return Peers<T>{reinterpret_cast<const T*>(c->peer_lo + off) + shift, reinterpret_cast<const T*>(c->peer_hi + off) - shift};
+}
+
 // The LB kernels can be launched on a range of owned planes [z0, z1) (inner / outer split of a slab,
 // Alg. 2 lines 4-10); the buffers flip when the step is committed.
 template <typename T>
@@ -171,6 +184,8 @@ static int launch_phase_range(acm_ctx* c, int z0, int z1)
     a.one_minus_omega = (T)(1.0 - omega);
     a.inv_xi = (T)(1.0 / c->xi);
     a.ref = (T)c->ref;
+    a.Hpeer = peers_at<T>(c, c->offH[c->curH]);
+    a.Cpeer = peers_at<T>(c, c->offC[c->curC]);
     const Launch l = lb_launch(c, z1 - z0);
     const int coll = (c->options & ACM_OPT_PHASE_SRT) ? PHASE_SRT : PHASE_MRT;
     const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
@@ -201,6 +216,8 @@ static int launch_hydro_range(acm_ctx* c, int z0, int z1)
     a.tau_L = (T)(3.0 * c->nu_L + c->ref * (3.0 * c->nu_H - 3.0 * c->nu_L)); a.dtau = (T)(3.0 * c->nu_H - 3.0 * c->nu_L);
     a.beta4 = (T)(4.0 * 12.0 * c->sigma / c->xi); a.kappa = (T)(1.5 * c->sigma * c->xi);
     a.gx = (T)c->grav[0]; a.gy = (T)c->grav[1]; a.gz = (T)c->grav[2];
+    a.Gpeer = peers_at<T>(c, c->offG[c->curG]);
+    a.Cpeer = peers_at<T>(c, c->offC[c->curC]);
     const Launch l = lb_launch(c, z1 - z0);
     const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
     cudaError_t e = unfused ? launch_unfused_hydro<T>(c->Qg, c->walls != 0, l, a, wsp<T>(c, c->offU[c->curU]), wsp<T>(c, c->offU[c->curU ^ 1]))
@@ -352,6 +369,7 @@ static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase,
         if (!slab || rank == nranks - 1) c->walls |= WALL_ZHI;
     }
     c->ref_mode = -1; c->ref = 0.0;
+    c->peer_on = false; c->peer_lo = c->peer_hi = nullptr;
     c->nzl = nzl; c->zlo = slab ? 1 : 0; c->ghost = slab ? 1 : 0;
     c->zglob0 = zglob0; c->nz_global = slab ? nz_global : nzl; c->rank = slab ? rank : 0; c->nranks = slab ? nranks : 1;
     c->stream = (cudaStream_t)cuda_stream;
@@ -486,6 +504,22 @@ int acm_halo_plan(const acm_ctx* c, int what, int side, int recv, int max_chunks
         bytes[k] = plane;
     }
     return n;
+}
+
+int acm_set_peers(acm_ctx* c, void* lo_workspace, void* hi_workspace)
+{
+    ACM_CHECK_CTX(c);
+    if (!c->ghost) return fail(ACM_ESTATE, "acm_set_peers: not a slab context");
+    if (!lo_workspace && !hi_workspace) { c->peer_on = false; c->peer_lo = c->peer_hi = nullptr; return ACM_OK; }
+    if (c->nz_global % c->nranks != 0) return fail(ACM_EINVAL, "acm_set_peers: needs slabs of equal height (nz_global %% nranks == 0)");
+    const bool need_lo = !((c->walls & WALL_ZLO) != 0), need_hi = !((c->walls & WALL_ZHI) != 0);
+    if ((need_lo && !lo_workspace) || (need_hi && !hi_workspace))
+        return fail(ACM_EINVAL, "acm_set_peers: a neighbour workspace is missing on a face that is not a wall");
+    // a face on a wall of the global domain has no neighbour; its pointer is never dereferenced
+    c->peer_lo = lo_workspace ? (char*)lo_workspace : c->ws;
+    c->peer_hi = hi_workspace ? (char*)hi_workspace : c->ws;
+    c->peer_on = true;
+    return ACM_OK;
 }
 
 int acm_phase_launch(acm_ctx* c, int z0, int z1)

@@ -55,6 +55,7 @@ struct Nbr {
     unsigned xs[3];        // x-1, x, x+1
     unsigned row[3][3];    // [dz+1][dy+1] -> (z'*ny + y')*nx
     bool wxm, wxp, wym, wyp, wzm, wzp;   // the cell at x-1 / x+1 / ... lies beyond a wall
+    bool peer_lo, peer_hi;               // slab: the plane z-1 / z+1 belongs to the low / high neighbour slab
 
     template <bool WALLS>
     __device__ __forceinline__ void setup(const Geom& g, int x, int y, int z)
@@ -68,6 +69,8 @@ struct Nbr {
         // z: wall -> clamp; ghost planes -> use them as they are; else periodic wrap inside [zlo, zhi)
         if (zm < g.zlo) { if (WALLS && (g.walls & WALL_ZLO)) { wzm = true; zm = g.zlo; } else if (!g.zghost) zm = g.zhi - 1; }
         if (zp >= g.zhi) { if (WALLS && (g.walls & WALL_ZHI)) { wzp = true; zp = g.zhi - 1; } else if (!g.zghost) zp = g.zlo; }
+        peer_lo = g.zghost && z == g.zlo && !wzm;
+        peer_hi = g.zghost && z == g.zhi - 1 && !wzp;
         xs[0] = (unsigned)xm; xs[1] = (unsigned)x; xs[2] = (unsigned)xp;
         const int ys[3] = {ym, y, yp}, zs[3] = {zm, z, zp};
 #pragma unroll
@@ -150,9 +153,19 @@ enum { ST_POST = 0, ST_IN = 1, ST_SWAP = 2 };
 // variants of the phase-field collision (ACM_OPT_PHASE_SRT)
 enum { PHASE_MRT = 0, PHASE_SRT = 1 };
 
+// Peer mode of a slab (acm_set_peers): what lies in the planes just outside the owned range is read straight from
+// the neighbour slabs' arrays -- device pointers into another context's workspace, on this GPU or mapped from a peer
+// GPU over NVLink -- instead of from ghost planes filled by an exchange.  `lo` / `hi` are the neighbours' arrays
+// shifted such that this slab's own cell index addresses the right plane (equal slab heights).
+template <typename T>
+struct Peers {
+    const T* lo;
+    const T* hi;
+};
+
 // incoming populations f_i(x) from an array in state STATE
-template <int Q, typename T, bool WALLS, int STATE>
-__device__ __forceinline__ void load_incoming(const T* F, size_t N, const Nbr& nb, T (&f)[Q])
+template <int Q, typename T, bool WALLS, int STATE, bool PEER = false>
+__device__ __forceinline__ void load_incoming(const T* F, size_t N, const Nbr& nb, T (&f)[Q], Peers<T> peers = Peers<T>{nullptr, nullptr})
 {
     using L = Lat<Q>;
     static_for<0, Q>([&](auto ic) {
@@ -164,7 +177,10 @@ __device__ __forceinline__ void load_incoming(const T* F, size_t N, const Nbr& n
         } else {
             constexpr int far = (STATE == ST_POST) ? i : o;      // slot at x - e_i
             constexpr int own = (STATE == ST_POST) ? o : i;      // slot at x when x - e_i is beyond a wall
-            src = F + (size_t)far * N + nb.template at<-ex, -ey, -ez>();
+            const T* base = F;
+            if constexpr (PEER && ez > 0) base = nb.peer_lo ? peers.lo : F;      // pulled from the plane z - 1
+            if constexpr (PEER && ez < 0) base = nb.peer_hi ? peers.hi : F;      // pulled from the plane z + 1
+            src = base + (size_t)far * N + nb.template at<-ex, -ey, -ez>();
             if constexpr (WALLS && i > 0) {
                 if (nb.template beyond<-ex, -ey, -ez, WALLS>()) src = F + (size_t)own * N + nb.template at<0, 0, 0>();
             }
@@ -240,11 +256,18 @@ __device__ __forceinline__ void fd_phi_acc(const Acc& acc, T c0, T& gx, T& gy, T
 
 // where the phi stencil reads from: global memory through L1/L2 (default), or a shared-memory tile of the
 // block's 3 x 3 neighbouring rows (the ACM_PHI_SMEM experiment, profiles/r1b_profiles.md)
-template <typename T>
+template <typename T, bool PEER = false>
 struct PhiGlobal {
     const T* C;
     const Nbr* nb;
-    template <int DX, int DY, int DZ> __device__ __forceinline__ T get() const { return __ldg(C + nb->template at<DX, DY, DZ>()); }
+    Peers<T> peers;
+    template <int DX, int DY, int DZ> __device__ __forceinline__ T get() const
+    {
+        const T* base = C;
+        if constexpr (PEER && DZ < 0) base = nb->peer_lo ? peers.lo : C;
+        if constexpr (PEER && DZ > 0) base = nb->peer_hi ? peers.hi : C;
+        return __ldg(base + nb->template at<DX, DY, DZ>());
+    }
 };
 template <typename T>
 struct PhiTile {
@@ -256,7 +279,13 @@ struct PhiTile {
 template <int Q, typename T, bool LAPLACE>
 __device__ __forceinline__ void fd_phi(const T* __restrict__ C, const Nbr& nb, T c0, T& gx, T& gy, T& gz, T& lap)
 {
-    fd_phi_acc<Q, T, LAPLACE>(PhiGlobal<T>{C, &nb}, c0, gx, gy, gz, lap);
+    fd_phi_acc<Q, T, LAPLACE>(PhiGlobal<T>{C, &nb, Peers<T>{nullptr, nullptr}}, c0, gx, gy, gz, lap);
+}
+
+template <int Q, typename T, bool LAPLACE>
+__device__ __forceinline__ void fd_phi_peer(const T* __restrict__ C, const Nbr& nb, Peers<T> peers, T c0, T& gx, T& gy, T& gz, T& lap)
+{
+    fd_phi_acc<Q, T, LAPLACE>(PhiGlobal<T, true>{C, &nb, peers}, c0, gx, gy, gz, lap);
 }
 
 #ifdef ACM_PHI_SMEM
@@ -290,6 +319,7 @@ struct PhaseArgs {
     unsigned N;      // cells per population plane (< 2^31): 32 bits keep the plane offsets i*N one wide multiply
     T one_minus_omega, inv_xi;
     T ref;           // fp32 instance: reference phase of the deviation storage (0 or 1); 0 for fp64
+    Peers<T> Hpeer, Cpeer;   // peer mode of a slab (else unused)
 };
 
 template <typename T>
@@ -301,6 +331,7 @@ struct HydroArgs {
     unsigned N;      // cells per population plane (< 2^31): 32 bits keep the plane offsets i*N one wide multiply
     T rho_L, drho, tau_L, dtau, beta4, kappa, gx, gy, gz;
     T ref;           // as in PhaseArgs; rho_L, tau_L are the values at phi = ref
+    Peers<T> Gpeer, Cpeer;   // peer mode of a slab (else unused)
 };
 
 }  // namespace acm

@@ -13,7 +13,7 @@ namespace acm {
 //   g*_i = g^eq_i(u_new) + F_i/2 + (1 - s_nu) 4.5 w_i (e_ia e_ib - d_ab/3) Pi_ab,
 //   Pi = P - p*/3 I - u_new u_new^T;  F_mu = -tau s_nu (P - p*/3 I - u_old u_old^T) grad rho
 // ------------------------------------------------------------------------------------------
-template <typename T, int Q, bool WALLS, int STATE>
+template <typename T, int Q, bool WALLS, int STATE, bool PEER = false>
 __global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const HydroArgs<T> a)
 {
     int x, y, z;
@@ -37,7 +37,7 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const H
     const size_t N = a.N;      // zero-extended 32-bit value
 
     T g[Q];
-    load_incoming<Q, T, WALLS, STATE>(a.Gsrc, N, nb, g);
+    load_incoming<Q, T, WALLS, STATE, PEER>(a.Gsrc, N, nb, g, a.Gpeer);
     const T uox = a.U[idx], uoy = a.U[N + idx], uoz = a.U[2 * N + idx];
     const T c0 = __ldg(a.C + idx);
     T gpx, gpy, gpz, lap;
@@ -45,7 +45,8 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const H
     if (tiled) fd_phi_acc<Q, T, true>(PhiTile<T>{phi_tile, (int)blockDim.x + 2, (int)threadIdx.x}, c0, gpx, gpy, gpz, lap);
     else
 #endif
-    fd_phi<Q, T, true>(a.C, nb, c0, gpx, gpy, gpz, lap);
+    if constexpr (PEER) fd_phi_peer<Q, T, true>(a.C, nb, a.Cpeer, c0, gpx, gpy, gpz, lap);
+    else fd_phi<Q, T, true>(a.C, nb, c0, gpx, gpy, gpz, lap);
 
     Moments<Q, T, true> m;
     m.compute(g);
@@ -59,6 +60,10 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const H
 template <typename T, int Q, bool WALLS>
 static void launch_hydro_state(int state, const Launch& l, const HydroArgs<T>& a)
 {
+    if (a.Gpeer.lo) {      // peer mode of a slab: two-grid storage only
+        hydro_kernel<T, Q, WALLS, ST_POST, true><<<l.grid, l.block, 0, l.stream>>>(a);
+        return;
+    }
     if (state == ST_POST) hydro_kernel<T, Q, WALLS, ST_POST><<<l.grid, l.block, 0, l.stream>>>(a);
     else if (state == ST_IN) hydro_kernel<T, Q, WALLS, ST_IN><<<l.grid, l.block, 0, l.stream>>>(a);
     else hydro_kernel<T, Q, WALLS, ST_SWAP><<<l.grid, l.block, 0, l.stream>>>(a);

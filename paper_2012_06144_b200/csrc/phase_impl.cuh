@@ -11,7 +11,7 @@ namespace acm {
 //   (first-order moments relaxed with omega_phi, all others with 1) -> store h, phi_new.
 // With d = j - phi_new u + (theta/6) n:   h*_i = h^eq_i + F_i/2 + (1-omega_phi) 3 w_i e_i.d
 // ------------------------------------------------------------------------------------------
-template <typename T, int Q, bool WALLS, int STATE, int COLL>
+template <typename T, int Q, bool WALLS, int STATE, int COLL, bool PEER = false>
 __global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const PhaseArgs<T> a)
 {
     int x, y, z;
@@ -35,7 +35,7 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const P
     const size_t N = a.N;      // zero-extended 32-bit value
 
     T h[Q];
-    load_incoming<Q, T, WALLS, STATE>(a.Hsrc, N, nb, h);
+    load_incoming<Q, T, WALLS, STATE, PEER>(a.Hsrc, N, nb, h, a.Hpeer);
     const T ux = __ldg(a.U + idx), uy = __ldg(a.U + N + idx), uz = __ldg(a.U + 2 * N + idx);
     const T c0 = __ldg(a.Csrc + idx);
     T gx, gy, gz, lap_unused;
@@ -43,7 +43,8 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const P
     if (tiled) fd_phi_acc<Q, T, false>(PhiTile<T>{phi_tile, (int)blockDim.x + 2, (int)threadIdx.x}, c0, gx, gy, gz, lap_unused);
     else
 #endif
-    fd_phi<Q, T, false>(a.Csrc, nb, c0, gx, gy, gz, lap_unused);
+    if constexpr (PEER) fd_phi_peer<Q, T, false>(a.Csrc, nb, a.Cpeer, c0, gx, gy, gz, lap_unused);
+    else fd_phi<Q, T, false>(a.Csrc, nb, c0, gx, gy, gz, lap_unused);
 
     Moments<Q, T, false> m;
     m.compute(h);
@@ -65,6 +66,11 @@ static void launch_phase_coll(int collision, const Launch& l, const PhaseArgs<T>
 template <typename T, int Q, bool WALLS>
 static void launch_phase_state(int state, int collision, const Launch& l, const PhaseArgs<T>& a)
 {
+    if (a.Hpeer.lo) {      // peer mode of a slab: two-grid storage only
+        if (collision == PHASE_SRT) phase_kernel<T, Q, WALLS, ST_POST, PHASE_SRT, true><<<l.grid, l.block, 0, l.stream>>>(a);
+        else phase_kernel<T, Q, WALLS, ST_POST, PHASE_MRT, true><<<l.grid, l.block, 0, l.stream>>>(a);
+        return;
+    }
     if (state == ST_POST) launch_phase_coll<T, Q, WALLS, ST_POST>(collision, l, a);
     else if (state == ST_IN) launch_phase_coll<T, Q, WALLS, ST_IN>(collision, l, a);
     else launch_phase_coll<T, Q, WALLS, ST_SWAP>(collision, l, a);

@@ -316,3 +316,94 @@ class SlabRunner:
         for s in self.slabs:
             tot = [a + b for a, b in zip(tot, s.bubble_sums())]
         return tot
+
+
+class PeerSlabRunner(SlabRunner):
+    """Slabs in PEER MODE (acm_set_peers): the LB kernels read the neighbour slabs' boundary planes straight from
+    the neighbours' workspaces -- the same GPU, or a peer GPU's memory mapped over NVLink (CUDA IPC) -- so a step is
+    just  phase kernel, signal, hydro kernel, signal  with no halo copies, no pack / unpack and no inner / outer
+    split; what crosses NVLink per step are the loads of the 5 + 5 (+ 2 phi) boundary planes themselves.
+
+    `peer_ws[r]` = (uint8 tensor over slab r's workspace allocation, byte offset of its 256-byte-aligned base) for
+    the neighbours of the local slabs; `sync()` must order kernel n of every rank after kernel n-1 of its
+    neighbours (nothing to do when all slabs share one stream).  Slabs must have equal heights.
+    """
+
+    def __init__(self, slabs, nranks, wall_z, peer_ws, sync=None, group=None):
+        super().__init__(slabs, nranks, wall_z, group, overlap=False)
+        self.peer_ws = dict(peer_ws)
+        self.sync = sync if sync is not None else (lambda: None)
+        self._wall_z = wall_z
+        for s in self.slabs:
+            lo, hi = self._neighbours(s.rank)
+            s._call(s._lib.acm_set_peers, self._ptr(lo), self._ptr(hi))
+
+    def _neighbours(self, r):
+        lo = None if (self._wall_z and r == 0) else (r - 1) % self.nranks
+        hi = None if (self._wall_z and r == self.nranks - 1) else (r + 1) % self.nranks
+        return lo, hi
+
+    def _ptr(self, r):
+        if r is None:
+            return None
+        t, base = self.peer_ws[r]
+        return C.c_void_p(t.data_ptr() + base)
+
+    @classmethod
+    def local(cls, p, nranks: int, precision="f64", device="cuda:0"):
+        slabs = [SlabACM(p, r, nranks, precision, device) for r in range(nranks)]
+        return cls(slabs, nranks, bool(p.wall_flags & binding.ACM_WALL_Z), {s.rank: (s.workspace, s.base) for s in slabs})
+
+    @classmethod
+    def distributed(cls, p, rank: int, world: int, precision="f64", device="cuda:0", group=None, sync=None):
+        """One slab per process.  The workspaces are shared through CUDA IPC (torch's own tensor sharing), gathered
+        with all_gather_object; default `sync`: a one-element all-reduce on the compute stream (NCCL), which makes
+        every rank's next kernel wait for all ranks' previous kernel without blocking the host."""
+        import torch.distributed as dist
+        from torch.multiprocessing.reductions import reduce_tensor
+        slab = SlabACM(p, rank, world, precision, device)
+        mine = (reduce_tensor(slab.workspace), slab.base)
+        gathered = [None] * world
+        dist.all_gather_object(gathered, mine, group=group)
+        peer_ws = {rank: (slab.workspace, slab.base)}
+        for r in {(rank - 1) % world, (rank + 1) % world} - {rank}:
+            (rebuild, args), base = gathered[r]
+            peer_ws[r] = (rebuild(*args), base)
+        if sync is None:
+            token = torch.zeros(1, device=device)
+
+            def sync():
+                dist.all_reduce(token, group=group)
+        return cls([slab], world, bool(p.wall_flags & binding.ACM_WALL_Z), peer_ws, sync, group)
+
+    # ---- a step: two kernels, two signals -----------------------------------------------------------------------
+    def step(self, n: int = 1):
+        for _ in range(int(n)):
+            for s in self.slabs:
+                s.phase_launch(0, s.nzl)
+                s.phase_commit()
+            self.sync()
+            for s in self.slabs:
+                s.hydro_launch(0, s.nzl)
+                s.hydro_commit()
+            self.sync()
+            self.steps += 1
+
+    def refresh_halos(self):
+        """Ghost planes are not used for stepping in peer mode; the exports (acm_get_pdfs, pressure) still read them:
+        pull them from the neighbours' workspaces.  Equal layouts: the neighbour's planes sit at the offsets of this
+        slab's own plan for the opposite face."""
+        self.sync()
+        for s in self.slabs:
+            lo, hi = self._neighbours(s.rank)
+            for what in (HALO_PHI, HALO_H, HALO_G):
+                for nb, my_side, nb_side in ((lo, 0, 1), (hi, 1, 0)):
+                    if nb is None:
+                        continue
+                    t, base = self.peer_ws[nb]
+                    for dst, (off, nbytes) in zip(s.halo_views(what, my_side, True), halo_plan(s._lib, s._h, what, nb_side, False)):
+                        dst.copy_(t[base + off: base + off + nbytes], non_blocking=True)
+        self.sync()
+
+    def sync_halos(self):
+        self.refresh_halos()

@@ -135,3 +135,102 @@ def test_slab_fp32_and_state_errors():
     with pytest.raises(AcmError) as e:
         r.slabs[0].step(1)
     assert e.value.code == ACM_ESTATE
+
+
+# ------------------------------------------------------------------------------------------------------------
+# peer mode: the kernels read the neighbour slabs' boundary planes directly (acm_set_peers), no halo copies
+# ------------------------------------------------------------------------------------------------------------
+def _peer_runner(p, nranks, **kw):
+    from paper_2012_06144_b200.slab import PeerSlabRunner
+    return PeerSlabRunner.local(p, nranks, **kw)
+
+
+@pytest.mark.parametrize("nranks", [1, 2, 3, 4])
+@pytest.mark.parametrize("nx,ny,nz,Qh,Qg,walls,srt", [(70, 6, 12, 15, 19, 0, False), (33, 5, 12, 27, 27, inputs.WALL_Y, True),
+                                                      (40, 4, 12, 19, 27, inputs.WALL_Z | inputs.WALL_X, False), (128, 3, 24, 15, 15, 0, False)])
+def test_peer_mode_steps_match_oracle_and_single_domain(nx, ny, nz, Qh, Qg, walls, srt, nranks):
+    p = Params(nx=nx, ny=ny, nz=nz, stencil_phase=Qh, stencil_hydro=Qg, wall_flags=walls, gravity=(1e-5, -1e-5, 2e-5),
+               nu_H=0.02, nu_L=0.05, phase_srt=srt)
+    phi, u, h, g = random_state(p, seed=43)
+    o = Oracle.from_params(p)
+    o.init(phi, u)
+    o.set_pdfs(h, g)
+    a = _acm(p)
+    a.init(_dev(phi), _dev(u))
+    a.set_pdfs(_dev(h), _dev(g))
+    r = _peer_runner(p, nranks)
+    r.init(_dev(phi), _dev(u))
+    r.set_pdfs(_dev(h), _dev(g))
+    for _ in range(3):
+        o.step(1)
+        a.step(1)
+        r.step(1)
+        ho, go = o.get_pdfs()
+        hr, gr = r.get_pdfs()
+        ha, ga = a.get_pdfs()
+        po, uo, pro = o.fields()
+        pr, ur, prr = r.fields()
+        pa, ua, pra = a.fields()
+        assert np.abs(hr.cpu().numpy() - ho).max() <= 1e-13
+        assert np.abs(gr.cpu().numpy() - go).max() <= 1e-13
+        assert np.abs(ur.cpu().numpy() - uo).max() <= 1e-13
+        assert np.abs(prr.cpu().numpy() - pro).max() <= 1e-13
+        for x, y in ((hr, ha), (gr, ga), (pr, pa), (ur, ua), (prr, pra)):
+            assert torch.equal(x, y)
+
+
+def test_peer_mode_never_reads_ghost_planes_while_stepping():
+    """poison the ghost planes of every array: the steps must not notice (ghosts are only refreshed for the exports)"""
+    p, phi, u = inputs.scaled_config3(24)
+    a = _acm(p)
+    a.init(_dev(phi), _dev(u))
+    r = _peer_runner(p, 3)
+    r.init(_dev(phi), _dev(u))
+    from paper_2012_06144_b200.slab import HALO_G, HALO_H, HALO_PHI
+    for k in range(4):
+        for s in r.slabs:
+            for what in (HALO_PHI, HALO_H, HALO_G):
+                for side in (0, 1):
+                    for v in s.halo_views(what, side, True):
+                        v.view(torch.float64).fill_(float("nan"))
+        r.step(1)
+        a.step(1)
+    for x, y in zip(r.get_pdfs() + r.fields(), a.get_pdfs() + a.fields()):
+        assert torch.equal(x, y)
+
+
+def test_peer_mode_100_steps_fp32_and_argument_checks():
+    from paper_2012_06144_b200.binding import AcmError, ACM_EINVAL
+    from paper_2012_06144_b200.slab import PeerSlabRunner
+    p = Params(nx=40, ny=6, nz=10, stencil_phase=27, stencil_hydro=27)
+    with pytest.raises(AcmError) as e:
+        PeerSlabRunner.local(p, 3)                       # 10 planes over 3 slabs: unequal heights
+    assert e.value.code == ACM_EINVAL
+    p, phi, u = inputs.scaled_config3(40)
+    o = Oracle.from_params(p)
+    o.init(phi, u)
+    r = _peer_runner(p, 4)
+    r.init(_dev(phi), _dev(u))
+    m0 = r.phi_mass_local()
+    o.step(100)
+    r.step(100)
+    po, uo, pro = o.fields()
+    pr, ur, prr = r.fields()
+    assert np.abs(pr.cpu().numpy() - po).max() <= 1e-10
+    assert np.abs(ur.cpu().numpy() - uo).max() <= 1e-10
+    assert abs(r.phi_mass_local() - m0) / m0 < 1e-12
+    # fp32 slabs in peer mode against the fp32 single domain (reference phase: heavy for slabs; force the same)
+    q = Params(nx=40, ny=6, nz=8, stencil_phase=15, stencil_hydro=19)
+    phi, u, h, g = random_state(q, seed=4)
+    phi, u, h, g = (np.asarray(x, dtype=np.float32) for x in (phi, u, h, g))
+    a = _acm(q, precision="f32")
+    a.set_reference_phase(1)
+    a.init(_dev(phi), _dev(u))
+    a.set_pdfs(_dev(h), _dev(g))
+    r = _peer_runner(q, 2, precision="f32")
+    r.init(_dev(phi), _dev(u))
+    r.set_pdfs(_dev(h), _dev(g))
+    a.step(3)
+    r.step(3)
+    for x, y in zip(r.get_pdfs(), a.get_pdfs()):
+        assert torch.equal(x, y)
