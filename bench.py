@@ -299,7 +299,7 @@ def run_decomposed(args, rank, local_rank, world):
     exchange halo planes every step (slab.py).  Not the default: `--gpus N` alone runs replicas."""
     import torch
     from paper_2012_06144_b200 import replicas
-    from paper_2012_06144_b200.slab import SlabRunner, pad_planes
+    from paper_2012_06144_b200.slab import PeerSlabRunner, SlabRunner, pad_planes
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
@@ -316,7 +316,11 @@ def run_decomposed(args, rank, local_rank, world):
     phi_h = torch.from_numpy(phi.astype(np_dtype)).pin_memory()
     u_h = torch.from_numpy(u.astype(np_dtype)).pin_memory()
     pg = p.replace(nz=p.nz * world)
-    run = SlabRunner.distributed(pg, rank, world, precision=precision, device=dev, overlap=not args.no_overlap)
+    if args.peer:       # the kernels read the neighbours' boundary planes directly (CUDA IPC / NVLink peer memory)
+        run = (PeerSlabRunner.local(pg, 1, precision=precision, device=dev) if world == 1
+               else PeerSlabRunner.distributed(pg, rank, world, precision=precision, device=dev))
+    else:
+        run = SlabRunner.distributed(pg, rank, world, precision=precision, device=dev, overlap=not args.no_overlap)
     slab = run.slabs[0]
 
     def load():
@@ -360,8 +364,9 @@ def run_decomposed(args, rank, local_rank, world):
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": precision, "data": "synthetic",
                "config": {"workload": name + f", stacked {world}x along z and decomposed into {world} z-slabs",
                           "grid": [pg.nx, pg.ny, pg.nz], "stencils": [p.stencil_phase, p.stencil_hydro],
-                          "parallelism": f"slab decomposition, {world} rank(s), halo exchange " +
-                                         ("overlapped on a second stream" if run.comm is not None else "in stream order"),
+                          "parallelism": f"slab decomposition, {world} rank(s), " +
+                                         ("peer mode: kernels read the neighbours' planes directly, one signal per kernel" if args.peer else
+                                          "halo exchange " + ("overlapped on a second stream" if run.comm is not None else "in stream order")),
                           "l2": "inputs larger than L2 (per rank as in the single-GPU run)",
                           "bytes_per_cell": {"phase": b_phase, "hydro": b_hydro}, "sum_phi_rank0": mass},
                "clocks": clk.summary(),
@@ -389,6 +394,7 @@ def main():
     ap.add_argument("--inplace", action="store_true", help="in-place AA streaming (one grid per population set)")
     ap.add_argument("--unfused", action="store_true", help="Algorithm 1 (six kernels per step) as a measured comparison")
     ap.add_argument("--decompose", action="store_true", help="one global domain in z-slabs with halo exchange instead of replicas")
+    ap.add_argument("--peer", action="store_true", help="with --decompose: peer mode (no halo copies; kernels read neighbour memory)")
     ap.add_argument("--no-overlap", action="store_true", help="with --decompose: exchange in stream order (no second stream)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
