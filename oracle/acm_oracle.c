@@ -37,12 +37,16 @@
  *   A19 p = p* rho c_s^2
  *   A23 variant ORACLE_VAR_PHASE_SRT: Omega^h = omega_phi I
  *   A24 bubble volume/centroid/velocity over phi < 1/2, weighted with 1 - phi
+ *   A25 two-dimensional instance: D2Q9 for both LB steps on one plane
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): lattice identities, weighted
  * orthogonality of M, eq.25 forcing identity, brute-force 4^3 step against a
  * hand-expanded projector form, FD operators on polynomials, sum(phi)
  * conservation, uniform state, Galilean invariance, planar tanh profile
- * (eq. 3), mobility and viscosity decay rates, Poiseuille profile, Laplace law.
+ * (eq. 3), mobility and viscosity decay rates, Poiseuille profile, Laplace law;
+ * variants (tests/test_oracle_variants.py, test_oracle_d2q9.py): SRT brute force and omega = 1
+ * special case, bubble diagnostics (symmetry, translation, continuum volume), eqs. 31-35
+ * round trip, D2Q9 lattice identities / brute force / transport limits.
  * Unpinned: rising-bubble drag/shape (eqs. 31-35; data only in figures).
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).
