@@ -98,8 +98,12 @@ int acm_create(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int ste
  *                     phi, collide h, stream g, update u, collide g) instead of two.  Same results as
  *                     the default (Algorithm 2); every population array is read three times and
  *                     written twice per step.  Needs 3N more workspace (u is double-buffered); cannot
- *                     be combined with ACM_OPT_INPLACE (ACM_EINVAL). */
-enum { ACM_OPT_INPLACE = 1, ACM_OPT_PHASE_SRT = 2, ACM_OPT_UNFUSED = 4, ACM_OPT_ALL = 7 };
+ *                     be combined with ACM_OPT_INPLACE (ACM_EINVAL).
+ *   ACM_OPT_BULK_ONE  the other reading of "we relax the second order moments with s_nu ... all other moments are
+ *                     relaxed by one" (A4/A26): only the five deviatoric second-order
+ *                     moments relax with s_nu, their trace (the bulk moment) with 1.  Same shear viscosity,
+ *                     bulk viscosity 1/9 instead of 2 nu/3.  Not with ACM_OPT_UNFUSED or slabs (ACM_EINVAL). */
+enum { ACM_OPT_INPLACE = 1, ACM_OPT_PHASE_SRT = 2, ACM_OPT_UNFUSED = 4, ACM_OPT_BULK_ONE = 8, ACM_OPT_ALL = 15 };
 size_t acm_workspace_bytes_opt(int nx, int ny, int nz, int stencil_phase, int stencil_hydro, int precision,
                                unsigned options);
 /* acm_create with options; acm_create(...) == acm_create_opt(..., options = 0, ...). */
@@ -110,8 +114,18 @@ int acm_create_opt(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int
 
 /* Equilibrium initialiser ("Initialisation of all fields", Alg. 2 line 1):
  * phi-field <- phi, u-field <- u, h_i <- phi Gamma_i(u) (eq. 6), g_i <- Gamma_i(u) - w_i
- * (eq. 12 with p* = 0).  phi: [device] N values; u: [device] 3N values, component-major. */
+ * (eq. 12 with p* = 0).  phi: [device] N values; u: [device] 3N values, component-major.
+ * Asynchronous, with one exception: for ACM_F32 with the automatic reference phase (acm_set_reference_phase = -1, the
+ * default, on a context that is not a slab) the call reduces mean(phi) on the device and SYNCHRONISES the stream to
+ * read it before it launches the initialiser. */
 int acm_init(acm_ctx*, const void* phi, const void* u);
+
+/* Velocity of eq. 22 by `sweeps` >= 1 sweeps of the fixed point u <- sum_i g_i e_i + F(u)/(2 rho): eq. 22 is implicit
+ * because the viscous force (eq. 18) contains g^eq(u).  sweeps = 1 (default, A10): F_mu is
+ * evaluated once with the velocity of the previous time step; sweeps = k re-evaluates it k-1 times with the velocity
+ * just obtained (A27).  Takes effect from the next step.  ACM_EINVAL for sweeps outside 1..64, or > 1 on a
+ * slab / with ACM_OPT_UNFUSED. */
+int acm_set_subiter(acm_ctx*, int sweeps);
 
 /* ACM_F32 only (no effect for ACM_F64).  The fp32 instance stores h_i - ref w_i and phi - ref instead of h_i and
  * phi, where ref = 0 (light) or 1 (heavy) is a reference phase: the bulk of that phase then keeps all its digits
@@ -125,6 +139,15 @@ int acm_set_reference_phase(acm_ctx*, int phase);
 /* Advances n >= 0 time steps (phase-field kernel, then hydrodynamic kernel, per step).
  * Asynchronous.  ACM_ESTATE before acm_init. */
 int acm_step(acm_ctx*, int n);
+
+/* CUDA graphs for launch-bound grids.  On a small grid (config 1: 32^3) a kernel is as short as its launch; acm_step
+ * then replays an executable graph of 16 consecutive steps (32 kernels; the buffer parity of the two-grid layout and
+ * the even/odd kernels of the in-place pattern repeat with period 2) and launches only the remaining n mod 16 steps
+ * one by one.  The graph is captured on a private stream on first use and launched on the context's stream; results
+ * are bit-identical to plain launches.  mode = -1 (default): automatic, for grids of at most 2^18 cells; 0: never;
+ * 1: always.  Never used while acm_profile is on or on slabs.  acm_graph_replays: graph launches so far. */
+int acm_set_graph(acm_ctx*, int mode);
+long long acm_graph_replays(const acm_ctx*);
 
 /* Copies out the macroscopic fields of the current time level: phi (N), u (3N, as stored by
  * the last hydrodynamic step, eq. 22) and the pressure p = p* rho(phi) c_s^2 with
@@ -224,7 +247,10 @@ int acm_set_peers(acm_ctx*, void* lo_workspace, void* hi_workspace);
 
 /* Launch one LB kernel on the owned planes [z0, z1) (0 <= z0 <= z1 <= owned planes; empty range = no launch)
  * without flipping the buffers; the *_commit call flips them once all planes of the step are launched.
- * Also valid on a plain context, where acm_step(1) equals launch(0, nz), commit for both kernels. */
+ * Also valid on a plain context, where acm_step(1) equals launch(0, nz), commit for both kernels.
+ * The inner / outer order of Alg. 2 is guarded: ACM_ESTATE for a commit unless exactly the owned planes
+ * were launched since the last commit of that kernel, for a launch that would exceed them, and for a launch of one
+ * kernel while the step of the other is partly launched. */
 int acm_phase_launch(acm_ctx*, int z0, int z1);
 int acm_phase_commit(acm_ctx*);
 int acm_hydro_launch(acm_ctx*, int z0, int z1);
@@ -246,13 +272,14 @@ int acm_set_pdfs(acm_ctx*, const void* h, const void* g);
 int acm_run_host(acm_ctx*, const void* phi_host, const void* u_host, int n,
                  void* phi_out_host, void* u_out_host, void* p_out_host);
 
-/* Launch geometry of the two LB kernels (threads per block along x, y, z; product <= 1024).
- * Optional; the defaults are tuned for B200. */
+/* Launch geometry of the two LB kernels (threads per block along x, y, z; product <= 256).
+ * Optional; the defaults are tuned for B200.  ACM_ESTATE while a step is partly launched. */
 int acm_set_block(acm_ctx*, int bx, int by, int bz);
 
 /* Per-kernel device timing for the roofline report.  acm_profile(ctx, 1) makes every later
  * acm_step record CUDA events on the stream around each of its two kernels (and drops earlier
- * records); acm_profile(ctx, 0) switches that off.  acm_profile_read synchronises the stream,
+ * records; the events are created before the first kernel of the call, not between kernels);
+ * acm_profile(ctx, 0) switches that off.  acm_profile_read synchronises the stream,
  * returns the summed durations in milliseconds of the phase-field and the hydrodynamic kernel
  * and the number of steps they cover, and clears the records.  Pointers are [host], may be NULL. */
 int acm_profile(acm_ctx*, int enable);

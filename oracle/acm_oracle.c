@@ -38,6 +38,12 @@
  *   A23 variant ORACLE_VAR_PHASE_SRT: Omega^h = omega_phi I
  *   A24 bubble volume/centroid/velocity over phi < 1/2, weighted with 1 - phi
  *   A25 two-dimensional instance: D2Q9 for both LB steps on one plane
+ *   A26 variant ORACLE_VAR_BULK_ONE: the trace of the second-order moments ("bulk" moment
+ *       x^2+y^2+z^2) counts among "all other moments" and relaxes with 1; the five deviatoric
+ *       second-order moments keep s_nu (the other reading of P:152-156, cf. A4)
+ *   A27 variant oracle_set_subiter(k): eq. 22 is implicit in F_mu (P:158 with eq. 18);
+ *       k fixed-point sweeps u <- sum g e + F(u)/(2 rho), F_mu re-evaluated with g^eq(u);
+ *       k = 1 is reading A10
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): lattice identities, weighted
  * orthogonality of M, eq.25 forcing identity, brute-force 4^3 step against a
@@ -46,7 +52,11 @@
  * (eq. 3), mobility and viscosity decay rates, Poiseuille profile, Laplace law;
  * variants (tests/test_oracle_variants.py, test_oracle_d2q9.py): SRT brute force and omega = 1
  * special case, bubble diagnostics (symmetry, translation, continuum volume), eqs. 31-35
- * round trip, D2Q9 lattice identities / brute force / transport limits.
+ * round trip, D2Q9 lattice identities / brute force / transport limits; A26: brute force with the
+ * projector split into deviatoric and trace parts, identical to the default at s_nu = 1, shear
+ * viscosity unchanged, sound attenuation changed as the bulk viscosity predicts; A27: k = 1 is the
+ * default bit for bit, the converged u satisfies eq. 22 to rounding (residual from a brute-force F).
+ * Two-phase flow: layered Poiseuille (F_mu) and two-layer hydrostatics (F_p), test_oracle_twophase.py.
  * Unpinned: rising-bubble drag/shape (eqs. 31-35; data only in figures).
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).
@@ -77,6 +87,8 @@ static const int DIRS27[27][3] = {
     {1, 1, 1}, {-1, -1, -1}, {1, 1, -1}, {-1, -1, 1},
     {1, -1, 1}, {-1, 1, -1}, {-1, 1, 1}, {1, -1, -1}};
 
+#define ORDER_BULK 20            /* row generated by x^2+y^2+z^2 when the bulk moment is split off (A26) */
+
 typedef struct {
     int Q;
     int e[QMAX][3];
@@ -97,12 +109,16 @@ typedef struct oracle_ctx {
     double *H, *H2, *G, *G2, *C, *C2, *U, *U2, *tmp;
     int initialised;
     unsigned variant;         /* ORACLE_VAR_* */
+    int subiter;              /* sweeps of the fixed point of eq. 22 (A27); 1 = reading A10 */
 } oracle_ctx;
 
 /* Variants of the operators the paper itself uses elsewhere:
  *   ORACLE_VAR_PHASE_SRT  single-relaxation-time phase-field collision, Omega^h = omega_phi I
- *                         ("a D3Q15 SRT LB scheme for the interface tracking"), reading A23 */
-enum { ORACLE_VAR_PHASE_SRT = 1 };
+ *                         ("a D3Q15 SRT LB scheme for the interface tracking"), reading A23
+ *   ORACLE_VAR_BULK_ONE   hydrodynamic collision: the bulk moment (trace of the second-order moments)
+ *                         relaxes with 1 like the higher moments, only the deviatoric second-order
+ *                         moments with s_nu ("all other moments are relaxed by one"), reading A26 */
+enum { ORACLE_VAR_PHASE_SRT = 1, ORACLE_VAR_BULK_ONE = 2 };
 
 /* ------------------------------------------------------------------------- */
 /* Lattices and moment matrices                                               */
@@ -147,18 +163,25 @@ static double ipow(int b, int p) { double r = 1.0; for (int k = 0; k < p; ++k) r
  * order of total degree; <p,q> = sum_i w_i p_i q_i ("weighted orthogonal moment
  * set").  Dependent monomials are dropped.  order[k] = degree of the
  * monomial that generated row k. */
-static int build_moments(lattice_t *L)
+/* bulk_split (A26): among the polynomials of degree 2 the trace x^2+y^2+z^2 is taken FIRST (row order
+ * ORDER_BULK); the monomials that follow then yield the deviatoric moments (the last one is dependent
+ * and dropped), all of them weighted-orthogonal to the bulk row. */
+static int build_moments(lattice_t *L, int bulk_split)
 {
     const int Q = L->Q;
     int rows = 0;
+    memset(L->M, 0, sizeof(L->M));
     for (int deg = 0; deg <= 6 && rows < Q; ++deg)
-        for (int a = 2; a >= 0; --a)
+        for (int a = (bulk_split && deg == 2) ? 3 : 2; a >= 0; --a)      /* a == 3 stands for the trace */
             for (int b = 2; b >= 0; --b)
                 for (int c = 2; c >= 0; --c) {
-                    if (a + b + c != deg || rows >= Q) continue;
+                    const int trace = (a == 3);
+                    if (trace && (b != 2 || c != 2)) continue;       /* one pass for the trace generator */
+                    if ((!trace && a + b + c != deg) || rows >= Q) continue;
                     double v[QMAX];
                     for (int i = 0; i < Q; ++i)
-                        v[i] = ipow(L->e[i][0], a) * ipow(L->e[i][1], b) * ipow(L->e[i][2], c);
+                        v[i] = trace ? (double)(L->e[i][0] * L->e[i][0] + L->e[i][1] * L->e[i][1] + L->e[i][2] * L->e[i][2])
+                                     : ipow(L->e[i][0], a) * ipow(L->e[i][1], b) * ipow(L->e[i][2], c);
                     /* two passes of Gram-Schmidt for numerical cleanliness */
                     for (int pass = 0; pass < 2; ++pass)
                         for (int r = 0; r < rows; ++r) {
@@ -174,7 +197,7 @@ static int build_moments(lattice_t *L)
                     for (int i = 0; i < Q; ++i) nrm += L->w[i] * v[i] * v[i];
                     if (nrm < 1e-12) continue;          /* linearly dependent on the lattice */
                     for (int i = 0; i < Q; ++i) L->M[rows * Q + i] = v[i];
-                    L->order[rows] = deg;
+                    L->order[rows] = trace ? ORDER_BULK : deg;
                     ++rows;
                 }
     if (rows != Q) return -1;
@@ -201,10 +224,10 @@ static int build_moments(lattice_t *L)
     return 0;
 }
 
-static int build_lattice(int Q, lattice_t *L)
+static int build_lattice(int Q, lattice_t *L, int bulk_split)
 {
     if (build_stencil(Q, L)) return -1;
-    return build_moments(L);
+    return build_moments(L, bulk_split);
 }
 
 /* Gamma_i(u), eq. 6 */
@@ -388,38 +411,44 @@ static void hydro_step(oracle_ctx *o)
                 double tau = o->tau_L + (phi - PHI_L) * (o->tau_H - o->tau_L);   /* eq. 20 */
                 double s_nu = 1.0 / (tau + 0.5);                                 /* eq. 21 */
                 double S[QMAX];
-                for (int k = 0; k < Q; ++k) S[k] = (L->order[k] == 2) ? s_nu : 1.0;          /* A4 */
+                /* A4: the six second-order moments relax with s_nu, all others with 1.  Variant A26: the
+                 * lattice was built with the bulk moment as a row of its own (order ORDER_BULK), which then
+                 * falls under "all others". */
+                for (int k = 0; k < Q; ++k) S[k] = (L->order[k] == 2) ? s_nu : 1.0;
 
-                /* H2: viscous force eq. 18 (A9, A10) with u of the previous step */
+                /* H2: viscous force eq. 18 (A9) with u of the previous step (A10); variant A27 repeats
+                 * H2 + H3 with the velocity just obtained (fixed point of eq. 22), o->subiter sweeps */
                 double uo[3] = {o->U[c], o->U[N + c], o->U[2 * N + c]};
                 double neq[QMAX], m[QMAX], v[QMAX];
-                for (int i = 0; i < Q; ++i) neq[i] = g[i] - (pstar * L->w[i] + Gamma(L, i, uo) - L->w[i]);  /* eq. 12 */
-                matvec(Q, L->M, neq, m);
-                for (int k = 0; k < Q; ++k) m[k] *= S[k];
-                matvec(Q, L->Minv, m, v);                                        /* Omega (g - geq) */
-                double nu = tau * CS2;                                           /* eq. 19 */
-                double Fmu[3];
-                for (int a = 0; a < 3; ++a) {
-                    double acc = 0.0;
-                    for (int b = 0; b < 3; ++b) {
-                        double Pi = 0.0;
-                        for (int k = 0; k < Q; ++k) Pi += L->e[k][a] * L->e[k][b] * v[k];
-                        acc += Pi * grho[b];
+                double F[3], un[3];
+                for (int sweep = 0; sweep < o->subiter; ++sweep) {
+                    for (int i = 0; i < Q; ++i) neq[i] = g[i] - (pstar * L->w[i] + Gamma(L, i, uo) - L->w[i]);  /* eq. 12 */
+                    matvec(Q, L->M, neq, m);
+                    for (int k = 0; k < Q; ++k) m[k] *= S[k];
+                    matvec(Q, L->Minv, m, v);                                        /* Omega (g - geq) */
+                    double nu = tau * CS2;                                           /* eq. 19 */
+                    double Fmu[3];
+                    for (int a = 0; a < 3; ++a) {
+                        double acc = 0.0;
+                        for (int b = 0; b < 3; ++b) {
+                            double Pi = 0.0;
+                            for (int k = 0; k < Q; ++k) Pi += L->e[k][a] * L->e[k][b] * v[k];
+                            acc += Pi * grho[b];
+                        }
+                        Fmu[a] = -(nu / CS2) * acc;
                     }
-                    Fmu[a] = -(nu / CS2) * acc;
-                }
-                double F[3];
-                for (int a = 0; a < 3; ++a)
-                    F[a] = mu * gphi[a]                       /* F_s, eq. 16 */
-                         - pstar * CS2 * grho[a]              /* F_p, eq. 14 */
-                         + Fmu[a]                             /* F_mu, eq. 18 */
-                         + rho * o->grav[a];                  /* F_b, eq. 30 (A17) */
-                /* H3: velocity, eq. 22 */
-                double un[3];
-                for (int a = 0; a < 3; ++a) {
-                    double j = 0.0;
-                    for (int i = 0; i < Q; ++i) j += g[i] * L->e[i][a];
-                    un[a] = j + F[a] / (2.0 * rho);
+                    for (int a = 0; a < 3; ++a)
+                        F[a] = mu * gphi[a]                       /* F_s, eq. 16 */
+                             - pstar * CS2 * grho[a]              /* F_p, eq. 14 */
+                             + Fmu[a]                             /* F_mu, eq. 18 */
+                             + rho * o->grav[a];                  /* F_b, eq. 30 (A17) */
+                    /* H3: velocity, eq. 22 */
+                    for (int a = 0; a < 3; ++a) {
+                        double j = 0.0;
+                        for (int i = 0; i < Q; ++i) j += g[i] * L->e[i][a];
+                        un[a] = j + F[a] / (2.0 * rho);
+                    }
+                    for (int a = 0; a < 3; ++a) uo[a] = un[a];
                 }
                 /* H4: collision in moment space, eq. 25 as in the listing P:229 (A6) */
                 double geq[QMAX], Fi[QMAX], meq[QMAX], Fm[QMAX], out[QMAX];
@@ -467,7 +496,8 @@ int oracle_create(oracle_ctx **out, int nx, int ny, int nz, int stencil_phase, i
     oracle_ctx *o = (oracle_ctx *)calloc(1, sizeof(oracle_ctx));
     if (!o) return 3;
     o->nx = nx; o->ny = ny; o->nz = nz; o->N = (size_t)nx * ny * nz;
-    if (build_lattice(stencil_phase, &o->Lh) || build_lattice(stencil_hydro, &o->Lg)) { free(o); return 1; }
+    if (build_lattice(stencil_phase, &o->Lh, 0) || build_lattice(stencil_hydro, &o->Lg, 0)) { free(o); return 1; }
+    o->subiter = 1;
     /* two-dimensional instance: both lattices D2Q9, one plane, no z component of gravity */
     if ((stencil_phase == 9) != (stencil_hydro == 9)) { free(o); return 1; }
     if (stencil_phase == 9 && (nz != 1 || (gravity && gravity[2] != 0.0))) { free(o); return 1; }
@@ -577,7 +607,9 @@ int oracle_set_pdfs(oracle_ctx *o, const double *h, const double *g)
 int oracle_lattice(int Q, int *e /*Q*3*/, double *w /*Q*/, int *opp, double *M /*Q*Q*/, double *Minv, int *order)
 {
     lattice_t L;
-    if (build_lattice(Q, &L)) return 1;
+    const int bulk_split = Q < 0;      /* -Q: the basis of variant A26 (bulk row has order ORDER_BULK) */
+    if (bulk_split) Q = -Q;
+    if (build_lattice(Q, &L, bulk_split)) return 1;
     for (int i = 0; i < Q; ++i) {
         if (e) { e[3 * i] = L.e[i][0]; e[3 * i + 1] = L.e[i][1]; e[3 * i + 2] = L.e[i][2]; }
         if (w) w[i] = L.w[i];
@@ -609,8 +641,18 @@ int oracle_fd(oracle_ctx *o, int use_hydro_stencil, const double *C, double *gra
 
 int oracle_set_variant(oracle_ctx *o, unsigned flags)
 {
-    if (!o || (flags & ~(unsigned)ORACLE_VAR_PHASE_SRT)) return 1;
+    if (!o || (flags & ~(unsigned)(ORACLE_VAR_PHASE_SRT | ORACLE_VAR_BULK_ONE))) return 1;
+    if ((flags ^ o->variant) & ORACLE_VAR_BULK_ONE)      /* the hydrodynamic moment basis with / without the bulk row */
+        if (build_lattice(o->Lg.Q, &o->Lg, (flags & ORACLE_VAR_BULK_ONE) != 0)) return 1;
     o->variant = flags;
+    return 0;
+}
+
+/* variant A27: number of sweeps of the fixed point of eq. 22 (1 = the default reading A10) */
+int oracle_set_subiter(oracle_ctx *o, int sweeps)
+{
+    if (!o || sweeps < 1 || sweeps > 64) return 1;
+    o->subiter = sweeps;
     return 0;
 }
 

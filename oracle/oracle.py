@@ -34,6 +34,7 @@ def _load():
         lib.oracle_fd.argtypes = [C.c_void_p, C.c_int, dp, dp, dp]
         lib.oracle_set_threads.argtypes = [C.c_int]
         lib.oracle_set_variant.argtypes = [C.c_void_p, C.c_uint]
+        lib.oracle_set_subiter.argtypes = [C.c_void_p, C.c_int]
         lib.oracle_bubble_diag.argtypes = [C.c_void_p, dp]
         lib.oracle_bubble_params.argtypes = [C.c_double] * 7 + [dp]
         lib.oracle_drag_lbm.argtypes = [C.c_double] * 5
@@ -52,8 +53,9 @@ def set_threads(n: int) -> int:
     return _load().oracle_set_threads(int(n))
 
 
-def lattice(Q: int):
-    """Direction table, weights, opposite index, moment matrix M, M^-1 and row orders."""
+def lattice(Q: int, bulk_split: bool = False):
+    """Direction table, weights, opposite index, moment matrix M, M^-1 and row orders.
+    bulk_split: the basis of variant A26 (the bulk moment is a row of its own, order ORDER_BULK)."""
     lib = _load()
     e = np.zeros((Q, 3), dtype=np.int32)
     w = np.zeros(Q)
@@ -62,14 +64,15 @@ def lattice(Q: int):
     Minv = np.zeros((Q, Q))
     order = np.zeros(Q, dtype=np.int32)
     ip = C.POINTER(C.c_int)
-    rc = lib.oracle_lattice(Q, e.ctypes.data_as(ip), _dp(w), opp.ctypes.data_as(ip), _dp(M), _dp(Minv),
+    rc = lib.oracle_lattice(-Q if bulk_split else Q, e.ctypes.data_as(ip), _dp(w), opp.ctypes.data_as(ip), _dp(M), _dp(Minv),
                             order.ctypes.data_as(ip))
     if rc:
         raise ValueError(f"unsupported stencil D3Q{Q}")
     return e, w, opp, M, Minv, order
 
 
-VAR_PHASE_SRT = 1
+VAR_PHASE_SRT, VAR_BULK_ONE = 1, 2
+ORDER_BULK = 20
 
 
 def bubble_params(Re_Gr, Eo, D, t_ref, rho_H=1.0, rho_star=1000.0, mu_star=100.0):
@@ -93,7 +96,8 @@ class Oracle:
     """Host-side twin of the acm_* call list."""
 
     def __init__(self, nx, ny, nz, stencil_phase=15, stencil_hydro=19, rho_H=1.0, rho_L=1e-3, sigma=1e-4, xi=5.0,
-                 M=0.02, nu_H=1 / 60, nu_L=1 / 60, gravity=(0.0, 0.0, 0.0), wall_flags=0, phase_srt=False):
+                 M=0.02, nu_H=1 / 60, nu_L=1 / 60, gravity=(0.0, 0.0, 0.0), wall_flags=0, phase_srt=False, bulk_one=False,
+                 subiter=1):
         self._lib = _load()
         self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
         self.Qh, self.Qg = int(stencil_phase), int(stencil_hydro)
@@ -106,8 +110,11 @@ class Oracle:
         if rc:
             raise ValueError(f"oracle_create failed with code {rc}")
         self._h = h
-        if phase_srt:
-            assert self._lib.oracle_set_variant(h, VAR_PHASE_SRT) == 0
+        flags = (VAR_PHASE_SRT if phase_srt else 0) | (VAR_BULK_ONE if bulk_one else 0)
+        if flags:
+            assert self._lib.oracle_set_variant(h, flags) == 0
+        if subiter != 1:
+            assert self._lib.oracle_set_subiter(h, int(subiter)) == 0
 
     @classmethod
     def from_params(cls, p, **kw):

@@ -15,11 +15,11 @@ from . import build as _build
 ACM_OK, ACM_EINVAL, ACM_ESTATE, ACM_ECUDA, ACM_EUNSTABLE = 0, 1, 2, 3, 4
 ACM_F64, ACM_F32 = 0, 1
 ACM_WALL_X, ACM_WALL_Y, ACM_WALL_Z = 1, 2, 4
-ACM_OPT_INPLACE, ACM_OPT_PHASE_SRT, ACM_OPT_UNFUSED = 1, 2, 4
+ACM_OPT_INPLACE, ACM_OPT_PHASE_SRT, ACM_OPT_UNFUSED, ACM_OPT_BULK_ONE = 1, 2, 4, 8
 
 EXPORTS = ["acm_workspace_bytes", "acm_workspace_bytes_opt", "acm_create", "acm_create_opt", "acm_init", "acm_step", "acm_fields", "acm_phi_mass", "acm_get_pdfs",
            "acm_set_pdfs", "acm_run_host", "acm_set_reference_phase", "acm_bubble_diag", "acm_bubble_sums", "acm_slab_range", "acm_workspace_bytes_slab", "acm_create_slab", "acm_slab_info",
-           "acm_halo_plan", "acm_set_peers", "acm_phase_launch", "acm_phase_commit", "acm_hydro_launch", "acm_hydro_commit", "acm_bubble_params", "acm_drag_lbm", "acm_drag_exp", "acm_set_block", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
+           "acm_halo_plan", "acm_set_peers", "acm_phase_launch", "acm_phase_commit", "acm_hydro_launch", "acm_hydro_commit", "acm_bubble_params", "acm_drag_lbm", "acm_drag_exp", "acm_set_block", "acm_set_subiter", "acm_set_graph", "acm_graph_replays", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
 
 _lib = None
 
@@ -80,6 +80,10 @@ def load(build_if_missing: bool = True):
     lib.acm_drag_exp.argtypes = [dbl]
     lib.acm_drag_exp.restype = dbl
     lib.acm_set_block.argtypes = [vp, i32, i32, i32]
+    lib.acm_set_subiter.argtypes = [vp, i32]
+    lib.acm_set_graph.argtypes = [vp, i32]
+    lib.acm_graph_replays.argtypes = [vp]
+    lib.acm_graph_replays.restype = C.c_longlong
     lib.acm_profile.argtypes = [vp, i32]
     lib.acm_profile_read.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(C.c_longlong)]
     lib.acm_launch_count.argtypes = [vp]
@@ -121,7 +125,8 @@ class ACM:
 
     def __init__(self, nx, ny, nz, stencil_phase=15, stencil_hydro=19, rho_H=1.0, rho_L=1e-3, sigma=1e-4, xi=5.0,
                  M=0.02, nu_H=1 / 60, nu_L=1 / 60, gravity=(0.0, 0.0, 0.0), wall_flags=0, precision="f64",
-                 device="cuda:0", stream=None, inplace=False, phase_srt=False, unfused=False, guard_bytes=0):
+                 device="cuda:0", stream=None, inplace=False, phase_srt=False, unfused=False, bulk_one=False, subiter=1,
+                 guard_bytes=0):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2012_06144_b200 needs a CUDA device (no CPU fallback)")
         self._lib = load()
@@ -133,7 +138,8 @@ class ACM:
         self.precision = {"f64": ACM_F64, "f32": ACM_F32}[precision]
         self.dtype = torch.float64 if precision == "f64" else torch.float32
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-        self.options = (ACM_OPT_INPLACE if inplace else 0) | (ACM_OPT_PHASE_SRT if phase_srt else 0) | (ACM_OPT_UNFUSED if unfused else 0)
+        self.options = ((ACM_OPT_INPLACE if inplace else 0) | (ACM_OPT_PHASE_SRT if phase_srt else 0) | (ACM_OPT_UNFUSED if unfused else 0)
+                        | (ACM_OPT_BULK_ONE if bulk_one else 0))
         nbytes = self._lib.acm_workspace_bytes_opt(self.nx, self.ny, self.nz, self.Qh, self.Qg, self.precision,
                                                    self.options)
         if nbytes == 0:
@@ -154,6 +160,8 @@ class ACM:
                                           C.c_void_p(base), C.c_void_p(self.stream.cuda_stream))
         _check(self._lib, rc)
         self._h = h
+        if subiter != 1:
+            self.set_subiter(subiter)
 
     @classmethod
     def from_params(cls, p, **kw):
@@ -185,6 +193,18 @@ class ACM:
 
     def set_block(self, bx, by=1, bz=1):
         self._call(self._lib.acm_set_block, int(bx), int(by), int(bz))
+
+    def set_subiter(self, sweeps):
+        """sweeps of the fixed point of eq. 22 (1 = single evaluation of F_mu with the previous velocity)"""
+        self._call(self._lib.acm_set_subiter, int(sweeps))
+
+    def set_graph(self, mode):
+        """CUDA graphs of 16 steps in acm_step: -1 automatic (small grids), 0 never, 1 always"""
+        self._call(self._lib.acm_set_graph, int(mode))
+
+    @property
+    def graph_replays(self):
+        return int(self._lib.acm_graph_replays(self._h))
 
     def set_reference_phase(self, phase):
         """fp32 instance: reference phase of the deviation storage (-1 automatic, 0 light, 1 heavy); before init"""

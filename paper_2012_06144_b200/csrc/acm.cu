@@ -60,11 +60,26 @@ struct acm_ctx {
     int sticky;                 // ACM_OK or ACM_ECUDA
     dim3 block;
     long long launches;
-    // optional per-kernel timing (acm_profile): events recorded around every LB kernel
+    int subiter;                // sweeps of the fixed point of eq. 22 (acm_set_subiter; 1 = the single evaluation, A10)
+    int phase_planes, hydro_planes;   // owned planes launched since the last acm_*_commit (guard of the split launches)
+    // optional per-kernel timing (acm_profile): events recorded around every LB kernel.  The events come from a pool
+    // that acm_step fills BEFORE its first launch, so that nothing but cudaEventRecord sits between two kernels.
     bool profiling;
-    std::vector<cudaEvent_t> ev;     // per acm_step call: e0 [phase] e1 [hydro] e2 [phase] ...
+    std::vector<cudaEvent_t> ev;     // pool; the first ev_used are recorded: per acm_step call e0 [phase] e1 [hydro] e2 [phase] ...
+    size_t ev_used;
     std::vector<int> ev_calls;       // number of steps of each recorded acm_step call
+    // CUDA graphs of GRAPH_STEPS consecutive steps for launch-bound (small) grids (acm_set_graph)
+    int graph_mode;                  // -1: automatic (grids of at most GRAPH_AUTO_CELLS cells), 0: never, 1: always
+    cudaStream_t cap_stream;         // private stream the steps are captured on (the caller's may be the legacy stream)
+    struct GraphEntry { unsigned key; cudaGraphExec_t exec; };
+    std::vector<GraphEntry> graphs;  // one per buffer / storage-state parity the capture started from
+    long long graph_replays;
 };
+
+// A graph holds an even number of steps: the buffer parity of the two-grid layout and the even/odd kernels of the
+// in-place pattern both repeat with period 2, so a replay leaves the host-side state as it found it.
+constexpr int GRAPH_STEPS = 16;
+constexpr size_t GRAPH_AUTO_CELLS = (size_t)1 << 18;     // 64^3: below this a kernel is as short as its launch
 
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
@@ -191,11 +206,13 @@ static int launch_phase_range(acm_ctx* c, int z0, int z1)
     const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
     cudaError_t e = unfused ? launch_unfused_phase<T>(c->Qh, c->walls != 0, coll, l, a)
                             : launch_phase<T>(c->Qh, c->walls != 0, c->stH, coll, l, a);
+    c->phase_planes += z1 - z0;
     return check_launch(c, unfused ? "stream_h/phi/collide_h kernels" : "phase_kernel", e, unfused ? 3 : 1);
 }
 
 static void commit_phase(acm_ctx* c)
 {
+    c->phase_planes = 0;
     c->curH ^= 1; c->curC ^= 1;
     c->stH = next_state(c->stH);
 }
@@ -216,17 +233,21 @@ static int launch_hydro_range(acm_ctx* c, int z0, int z1)
     a.tau_L = (T)(3.0 * c->nu_L + c->ref * (3.0 * c->nu_H - 3.0 * c->nu_L)); a.dtau = (T)(3.0 * c->nu_H - 3.0 * c->nu_L);
     a.beta4 = (T)(4.0 * 12.0 * c->sigma / c->xi); a.kappa = (T)(1.5 * c->sigma * c->xi);
     a.gx = (T)c->grav[0]; a.gy = (T)c->grav[1]; a.gz = (T)c->grav[2];
+    a.bulk_one = (c->options & ACM_OPT_BULK_ONE) ? 1 : 0;
+    a.subiter = c->subiter;
     a.Gpeer = peers_at<T>(c, c->offG[c->curG]);
     a.Cpeer = peers_at<T>(c, c->offC[c->curC]);
     const Launch l = lb_launch(c, z1 - z0);
     const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
     cudaError_t e = unfused ? launch_unfused_hydro<T>(c->Qg, c->walls != 0, l, a, wsp<T>(c, c->offU[c->curU]), wsp<T>(c, c->offU[c->curU ^ 1]))
                             : launch_hydro<T>(c->Qg, c->walls != 0, c->stG, l, a);
+    c->hydro_planes += z1 - z0;
     return check_launch(c, unfused ? "stream_g/velocity/collide_g kernels" : "hydro_kernel", e, unfused ? 3 : 1);
 }
 
 static void commit_hydro(acm_ctx* c)
 {
+    c->hydro_planes = 0;
     if (c->options & ACM_OPT_UNFUSED) c->curU ^= 1;
     c->curG ^= 1;
     c->stG = next_state(c->stG);
@@ -250,17 +271,75 @@ static int launch_hydro_step(acm_ctx* c)
 
 static void prof_mark(acm_ctx* c)
 {
-    if (!c->profiling) return;
-    cudaEvent_t e;
-    if (cudaEventCreate(&e) != cudaSuccess) return;
-    cudaEventRecord(e, c->stream);
-    c->ev.push_back(e);
+    if (!c->profiling || c->ev_used >= c->ev.size()) return;
+    cudaEventRecord(c->ev[c->ev_used++], c->stream);
+}
+
+// make sure the pool holds `count` unused events (created here, outside the kernel sequence)
+static bool prof_reserve(acm_ctx* c, size_t count)
+{
+    while (c->ev.size() < c->ev_used + count) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return false;
+        c->ev.push_back(e);
+    }
+    return true;
+}
+
+static void graphs_clear(acm_ctx* c)
+{
+    for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
+    c->graphs.clear();
+}
+
+static unsigned graph_key(const acm_ctx* c)
+{
+    return (unsigned)c->curH | (unsigned)c->curG << 1 | (unsigned)c->curC << 2 | (unsigned)c->curU << 3 | (unsigned)c->stH << 4 | (unsigned)c->stG << 6;
+}
+
+static bool graph_wanted(const acm_ctx* c)
+{
+    if (c->profiling || c->ghost) return false;
+    return c->graph_mode > 0 || (c->graph_mode < 0 && (size_t)c->nx * c->ny * c->nzl <= GRAPH_AUTO_CELLS);
+}
+
+template <typename T> static int plain_steps(acm_ctx* c, int n);
+
+// the executable graph of GRAPH_STEPS steps starting from the current buffer parity (captured on first use)
+template <typename T>
+static cudaGraphExec_t graph_for_state(acm_ctx* c)
+{
+    const unsigned key = graph_key(c);
+    for (auto& g : c->graphs)
+        if (g.key == key) return g.exec;
+    if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    const cudaStream_t user = c->stream;
+    const long long launches = c->launches;
+    c->stream = c->cap_stream;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    bool ok = cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+    if (ok) {
+        ok = plain_steps<T>(c, GRAPH_STEPS) == ACM_OK;      // recorded, not executed; the state is back where it was (even count)
+        ok = (cudaStreamEndCapture(c->cap_stream, &graph) == cudaSuccess) && ok && graph;
+    }
+    if (ok) ok = cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess;
+    if (graph) cudaGraphDestroy(graph);
+    c->stream = user;
+    c->launches = launches;
+    if (!ok) {
+        cudaGetLastError();
+        c->sticky = ACM_OK;          // a failed capture is not a failed launch: fall back to plain launches
+        c->graph_mode = 0;
+        return nullptr;
+    }
+    c->graphs.push_back({key, exec});
+    return exec;
 }
 
 template <typename T>
-static int step_t(acm_ctx* c, int n)
+static int plain_steps(acm_ctx* c, int n)
 {
-    if (c->profiling && n > 0) { c->ev_calls.push_back(n); prof_mark(c); }
     for (int t = 0; t < n; ++t) {
         int rc = launch_phase_step<T>(c);
         if (rc) return rc;
@@ -270,6 +349,30 @@ static int step_t(acm_ctx* c, int n)
         prof_mark(c);
     }
     return ACM_OK;
+}
+
+template <typename T>
+static int step_t(acm_ctx* c, int n)
+{
+    if (c->profiling && n > 0) {
+        if (!prof_reserve(c, 2 * (size_t)n + 1)) return fail(ACM_ECUDA, "acm_step: cudaEventCreate failed");
+        c->ev_calls.push_back(n);
+        prof_mark(c);
+    }
+    int done = 0;
+    if (graph_wanted(c)) {
+        const int per_step = (c->options & ACM_OPT_UNFUSED) ? 6 : 2;
+        while (n - done >= GRAPH_STEPS) {
+            cudaGraphExec_t exec = graph_for_state<T>(c);
+            if (!exec) break;
+            cudaError_t e = cudaGraphLaunch(exec, c->stream);
+            if (e != cudaSuccess) { c->sticky = ACM_ECUDA; return fail(ACM_ECUDA, "acm_step: cudaGraphLaunch: %s", cudaGetErrorString(e)); }
+            c->launches += (long long)per_step * GRAPH_STEPS;
+            c->graph_replays += 1;
+            done += GRAPH_STEPS;
+        }
+    }
+    return plain_steps<T>(c, n - done);
 }
 
 template <typename T>
@@ -335,9 +438,11 @@ static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase,
 {
     const bool slab = nranks > 0;
     const int nzl = nz;
+    if ((options & ACM_OPT_BULK_ONE) && (options & ACM_OPT_UNFUSED))
+        return fail(ACM_EINVAL, "acm_create: ACM_OPT_BULK_ONE is not available with ACM_OPT_UNFUSED");
     if (slab) {
-        if (options & (ACM_OPT_INPLACE | ACM_OPT_UNFUSED))
-            return fail(ACM_EINVAL, "acm_create_slab: ACM_OPT_INPLACE / ACM_OPT_UNFUSED are not available for slabs");
+        if (options & (ACM_OPT_INPLACE | ACM_OPT_UNFUSED | ACM_OPT_BULK_ONE))
+            return fail(ACM_EINVAL, "acm_create_slab: ACM_OPT_INPLACE / ACM_OPT_UNFUSED / ACM_OPT_BULK_ONE are not available for slabs");
         if (nz > 0) nz += 2;      // ghost planes below and above
     }
     if (!out) return fail(ACM_EINVAL, "acm_create: out is NULL");
@@ -385,7 +490,13 @@ static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase,
     // or 256 fp32 cells along x; fp32 falls back to 128 when nx is not a multiple of 256
     c->block = (precision == ACM_F32 && nx % 256 == 0) ? dim3(256, 1, 1) : dim3(128, 1, 1);
     c->launches = 0;
+    c->subiter = 1;
+    c->phase_planes = c->hydro_planes = 0;
     c->profiling = false;
+    c->ev_used = 0;
+    c->graph_mode = -1;
+    c->cap_stream = nullptr;
+    c->graph_replays = 0;
     *out = c;
     return ACM_OK;
 }
@@ -527,12 +638,16 @@ int acm_phase_launch(acm_ctx* c, int z0, int z1)
     ACM_CHECK_CTX(c);
     if (!c->initialised) return fail(ACM_ESTATE, "acm_phase_launch: call acm_init first");
     if (z0 < 0 || z1 > c->nzl || z0 > z1) return fail(ACM_EINVAL, "acm_phase_launch: need 0 <= z0 <= z1 <= owned planes");
+    if (c->phase_planes + (z1 - z0) > c->nzl) return fail(ACM_ESTATE, "acm_phase_launch: more planes than the slab owns since the last acm_phase_commit");
+    if (c->hydro_planes) return fail(ACM_ESTATE, "acm_phase_launch: the hydrodynamic step is not committed");
     return c->precision == ACM_F64 ? launch_phase_range<double>(c, z0, z1) : launch_phase_range<float>(c, z0, z1);
 }
 
 int acm_phase_commit(acm_ctx* c)
 {
     ACM_CHECK_CTX(c);
+    if (c->phase_planes != c->nzl)
+        return fail(ACM_ESTATE, "acm_phase_commit: %d of %d owned planes were launched since the last commit", c->phase_planes, c->nzl);
     commit_phase(c);
     return ACM_OK;
 }
@@ -542,27 +657,32 @@ int acm_hydro_launch(acm_ctx* c, int z0, int z1)
     ACM_CHECK_CTX(c);
     if (!c->initialised) return fail(ACM_ESTATE, "acm_hydro_launch: call acm_init first");
     if (z0 < 0 || z1 > c->nzl || z0 > z1) return fail(ACM_EINVAL, "acm_hydro_launch: need 0 <= z0 <= z1 <= owned planes");
+    if (c->hydro_planes + (z1 - z0) > c->nzl) return fail(ACM_ESTATE, "acm_hydro_launch: more planes than the slab owns since the last acm_hydro_commit");
+    if (c->phase_planes) return fail(ACM_ESTATE, "acm_hydro_launch: the phase-field step is not committed");
     return c->precision == ACM_F64 ? launch_hydro_range<double>(c, z0, z1) : launch_hydro_range<float>(c, z0, z1);
 }
 
 int acm_hydro_commit(acm_ctx* c)
 {
     ACM_CHECK_CTX(c);
+    if (c->hydro_planes != c->nzl)
+        return fail(ACM_ESTATE, "acm_hydro_commit: %d of %d owned planes were launched since the last commit", c->hydro_planes, c->nzl);
     commit_hydro(c);
     return ACM_OK;
 }
 
-static void prof_clear(acm_ctx* c)
+static void prof_clear(acm_ctx* c)      // forget the records, keep the pool
 {
-    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
-    c->ev.clear();
+    c->ev_used = 0;
     c->ev_calls.clear();
 }
 
 void acm_destroy(acm_ctx* c)
 {
     if (!c) return;
-    prof_clear(c);
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    graphs_clear(c);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     delete c;
 }
 
@@ -583,7 +703,7 @@ int acm_profile_read(acm_ctx* c, double* phase_ms, double* hydro_ms, long long* 
     long long ns = 0;
     size_t k = 0;
     for (int n : c->ev_calls) {
-        if (k + 2 * (size_t)n + 1 > c->ev.size()) break;
+        if (k + 2 * (size_t)n + 1 > c->ev_used) break;
         for (int t = 0; t < n; ++t) {
             float a = 0.f, b = 0.f;
             cudaEventElapsedTime(&a, c->ev[k + 2 * t], c->ev[k + 2 * t + 1]);
@@ -605,9 +725,33 @@ int acm_set_block(acm_ctx* c, int bx, int by, int bz)
     ACM_CHECK_CTX(c);
     if (bx < 1 || by < 1 || bz < 1 || (long long)bx * by * bz > 256 || bz > 64)
         return fail(ACM_EINVAL, "acm_set_block: need 1 <= bx*by*bz <= 256");
+    if (c->phase_planes || c->hydro_planes) return fail(ACM_ESTATE, "acm_set_block: a step is partly launched (commit it first)");
     c->block = dim3(bx, by, bz);
+    graphs_clear(c);
     return ACM_OK;
 }
+
+int acm_set_subiter(acm_ctx* c, int sweeps)
+{
+    ACM_CHECK_CTX(c);
+    if (sweeps < 1 || sweeps > 64) return fail(ACM_EINVAL, "acm_set_subiter: need 1 <= sweeps <= 64");
+    if (sweeps > 1 && (c->ghost || (c->options & ACM_OPT_UNFUSED)))
+        return fail(ACM_EINVAL, "acm_set_subiter: not available for slabs or with ACM_OPT_UNFUSED");
+    if (c->phase_planes || c->hydro_planes) return fail(ACM_ESTATE, "acm_set_subiter: a step is partly launched (commit it first)");
+    c->subiter = sweeps;
+    graphs_clear(c);
+    return ACM_OK;
+}
+
+int acm_set_graph(acm_ctx* c, int mode)
+{
+    ACM_CHECK_CTX(c);
+    if (mode < -1 || mode > 1) return fail(ACM_EINVAL, "acm_set_graph: mode must be -1 (automatic), 0 (never) or 1 (always)");
+    c->graph_mode = mode;
+    return ACM_OK;
+}
+
+long long acm_graph_replays(const acm_ctx* c) { return c ? c->graph_replays : 0; }
 
 long long acm_launch_count(const acm_ctx* c) { return c ? c->launches : 0; }
 
@@ -615,6 +759,8 @@ int acm_init(acm_ctx* c, const void* phi, const void* u)
 {
     ACM_CHECK_CTX(c);
     if (!phi || !u) return fail(ACM_EINVAL, "acm_init: phi and u are required");
+    graphs_clear(c);                  // the reference phase of the fp32 instance is a kernel argument
+    c->phase_planes = c->hydro_planes = 0;
     c->ref = 0.0;
     if (c->precision == ACM_F32) {
         // reference phase of the deviation storage: the phase that fills most of the domain

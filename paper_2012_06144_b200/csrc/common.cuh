@@ -97,13 +97,7 @@ struct Nbr {
     }
 };
 
-// tuning knobs (defaults = the measured best on B200)
-#ifndef ACM_LD
-#define ACM_LD 2
-#endif
-#ifndef ACM_ST
-#define ACM_ST 2
-#endif
+// launch bounds of the two LB kernels (the fp32 translation units raise the minimum blocks per SM)
 #ifndef ACM_PHASE_MINB
 #define ACM_PHASE_MINB 1
 #endif
@@ -114,28 +108,10 @@ struct Nbr {
 #define ACM_MAXT 256
 #endif
 
-// population loads/stores.  Measured on B200 (profiles/r1_variants.md): plain ld/st beat the
-// streaming hints (__ldcs/__stcs) by 5 % on the whole step, so plain is the default.
-template <typename T> __device__ __forceinline__ T ld_stream(const T* p)
-{
-#if ACM_LD == 0
-    return __ldcs(p);
-#elif ACM_LD == 1
-    return __ldg(p);
-#else
-    return *p;
-#endif
-}
-template <typename T> __device__ __forceinline__ void st_stream(T* p, T v)
-{
-#if ACM_ST == 0
-    __stcs(p, v);
-#elif ACM_ST == 1
-    __stcg(p, v);
-#else
-    *p = v;
-#endif
-}
+// population loads/stores: plain ld/st.  Measured on B200 (profiles/r1_variants.md): the streaming hints
+// (__ldcs/__stcs, __ldg/__stcg) lose 5 % on the whole step against plain accesses.
+template <typename T> __device__ __forceinline__ T ld_stream(const T* p) { return *p; }
+template <typename T> __device__ __forceinline__ void st_stream(T* p, T v) { *p = v; }
 
 // ------------------------------------------------------------------------------------------
 // Storage states of a population array and the streaming they imply.
@@ -254,8 +230,8 @@ __device__ __forceinline__ void fd_phi_acc(const Acc& acc, T c0, T& gx, T& gy, T
     if constexpr (LAPLACE) lap = l - T(6.0 * (1.0 - L::wc(0))) * c0;   // sum_{i>=1} w_i = 1 - w_0
 }
 
-// where the phi stencil reads from: global memory through L1/L2 (default), or a shared-memory tile of the
-// block's 3 x 3 neighbouring rows (the ACM_PHI_SMEM experiment, profiles/r1b_profiles.md)
+// the phi stencil reads global memory through L1/L2: ncu shows one DRAM read per phi value; a
+// shared-memory tile was measured 2-8 % slower (profiles/r1b_profiles.md) and is not kept
 template <typename T, bool PEER = false>
 struct PhiGlobal {
     const T* C;
@@ -269,13 +245,6 @@ struct PhiGlobal {
         return __ldg(base + nb->template at<DX, DY, DZ>());
     }
 };
-template <typename T>
-struct PhiTile {
-    const T* tile;     // [3][3][W]
-    int W, tx;
-    template <int DX, int DY, int DZ> __device__ __forceinline__ T get() const { return tile[((DZ + 1) * 3 + (DY + 1)) * W + tx + 1 + DX]; }
-};
-
 template <int Q, typename T, bool LAPLACE>
 __device__ __forceinline__ void fd_phi(const T* __restrict__ C, const Nbr& nb, T c0, T& gx, T& gy, T& gz, T& lap)
 {
@@ -287,25 +256,6 @@ __device__ __forceinline__ void fd_phi_peer(const T* __restrict__ C, const Nbr& 
 {
     fd_phi_acc<Q, T, LAPLACE>(PhiGlobal<T, true>{C, &nb, peers}, c0, gx, gy, gz, lap);
 }
-
-#ifdef ACM_PHI_SMEM
-// Cooperative load of the 9 rows (dy, dz in -1..1) of phi around the block's x-row, plus one halo cell on each
-// side, into shared memory.  Valid for 3-D launches with blocks of shape (bx, 1, 1): y and z are uniform per block.
-template <typename T>
-__device__ __forceinline__ void load_phi_tile(T* tile, const T* __restrict__ C, const Nbr& nb, int W, bool last_in_row)
-{
-    const int tx = threadIdx.x;
-#pragma unroll
-    for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = 0; b < 3; ++b) {
-            T* row = tile + (a * 3 + b) * W;
-            row[tx + 1] = __ldg(C + nb.row[a][b] + nb.xs[1]);
-            if (tx == 0) row[0] = __ldg(C + nb.row[a][b] + nb.xs[0]);
-            if (last_in_row) row[tx + 2] = __ldg(C + nb.row[a][b] + nb.xs[2]);
-        }
-}
-#endif
 
 // ------------------------------------------------------------------------------------------
 // argument blocks of the two LB kernels
@@ -331,6 +281,8 @@ struct HydroArgs {
     unsigned N;      // cells per population plane (< 2^31): 32 bits keep the plane offsets i*N one wide multiply
     T rho_L, drho, tau_L, dtau, beta4, kappa, gx, gy, gz;
     T ref;           // as in PhaseArgs; rho_L, tau_L are the values at phi = ref
+    int bulk_one;    // variant A26 (ACM_OPT_BULK_ONE): the bulk moment relaxes with 1; read by the HVAR = 1 instances only
+    int subiter;     // variant A27 (acm_set_subiter): sweeps of the fixed point of eq. 22, >= 1; HVAR = 1 instances only
     Peers<T> Gpeer, Cpeer;   // peer mode of a slab (else unused)
 };
 

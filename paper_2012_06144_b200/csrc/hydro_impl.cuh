@@ -13,26 +13,14 @@ namespace acm {
 //   g*_i = g^eq_i(u_new) + F_i/2 + (1 - s_nu) 4.5 w_i (e_ia e_ib - d_ab/3) Pi_ab,
 //   Pi = P - p*/3 I - u_new u_new^T;  F_mu = -tau s_nu (P - p*/3 I - u_old u_old^T) grad rho
 // ------------------------------------------------------------------------------------------
-template <typename T, int Q, bool WALLS, int STATE, bool PEER = false>
+// HVAR = 1: the operator variants of lb_math.cuh (bulk moment relaxed with 1, sub-iterated velocity), switched by a.bulk_one / a.subiter
+template <typename T, int Q, bool WALLS, int STATE, bool PEER = false, int HVAR = 0>
 __global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const HydroArgs<T> a)
 {
     int x, y, z;
-#ifdef ACM_PHI_SMEM
-    __shared__ T phi_tile[9 * (ACM_MAXT + 2)];
-    const bool active = cell_of_thread(a.g, x, y, z);
-    const bool tiled = !a.g.linear && blockDim.y == 1 && blockDim.z == 1;      // uniform over the block
-    Nbr nb;
-    if (active) nb.setup<WALLS>(a.g, x, y, z);
-    if (tiled) {
-        if (active) load_phi_tile<T>(phi_tile, a.C, nb, (int)blockDim.x + 2, threadIdx.x == blockDim.x - 1 || x == a.g.nx - 1);
-        __syncthreads();
-    }
-    if (!active) return;
-#else
     if (!cell_of_thread(a.g, x, y, z)) return;
     Nbr nb;
     nb.setup<WALLS>(a.g, x, y, z);
-#endif
     const unsigned idx = nb.at<0, 0, 0>();
     const size_t N = a.N;      // zero-extended 32-bit value
 
@@ -41,18 +29,14 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const H
     const T uox = a.U[idx], uoy = a.U[N + idx], uoz = a.U[2 * N + idx];
     const T c0 = __ldg(a.C + idx);
     T gpx, gpy, gpz, lap;
-#ifdef ACM_PHI_SMEM
-    if (tiled) fd_phi_acc<Q, T, true>(PhiTile<T>{phi_tile, (int)blockDim.x + 2, (int)threadIdx.x}, c0, gpx, gpy, gpz, lap);
-    else
-#endif
     if constexpr (PEER) fd_phi_peer<Q, T, true>(a.C, nb, a.Cpeer, c0, gpx, gpy, gpz, lap);
     else fd_phi<Q, T, true>(a.C, nb, c0, gpx, gpy, gpz, lap);
 
     Moments<Q, T, true> m;
     m.compute(g);
-    const HydroCell<T> hc = hydro_velocity<T, Q>(m, c0, gpx, gpy, gpz, lap, uox, uoy, uoz, a);
+    const HydroCell<T> hc = hydro_velocity<T, Q, HVAR>(m, c0, gpx, gpy, gpz, lap, uox, uoy, uoz, a);
     a.U[idx] = hc.ux; a.U[N + idx] = hc.uy; a.U[2 * N + idx] = hc.uz;
-    hydro_collide<T, Q>(m, hc, [&](auto ic, T v) {
+    hydro_collide<T, Q, HVAR>(m, hc, a, [&](auto ic, T v) {
         st_stream(outgoing_ptr<Q, decltype(ic)::value, T, WALLS, STATE>(a.Gdst, N, nb), v);
     });
 }
@@ -62,6 +46,12 @@ static void launch_hydro_state(int state, const Launch& l, const HydroArgs<T>& a
 {
     if (a.Gpeer.lo) {      // peer mode of a slab: two-grid storage only
         hydro_kernel<T, Q, WALLS, ST_POST, true><<<l.grid, l.block, 0, l.stream>>>(a);
+        return;
+    }
+    if (a.bulk_one || a.subiter > 1) {      // operator variants (not available in peer mode: acm.cu rejects the combination)
+        if (state == ST_POST) hydro_kernel<T, Q, WALLS, ST_POST, false, 1><<<l.grid, l.block, 0, l.stream>>>(a);
+        else if (state == ST_IN) hydro_kernel<T, Q, WALLS, ST_IN, false, 1><<<l.grid, l.block, 0, l.stream>>>(a);
+        else hydro_kernel<T, Q, WALLS, ST_SWAP, false, 1><<<l.grid, l.block, 0, l.stream>>>(a);
         return;
     }
     if (state == ST_POST) hydro_kernel<T, Q, WALLS, ST_POST><<<l.grid, l.block, 0, l.stream>>>(a);

@@ -99,7 +99,10 @@ struct HydroCell {
     T Sxx, Syy, Szz;   // P_aa - p*/3
 };
 
-template <typename T, int Q>
+// HVAR = 0: the default operators (readings A4, A10).  HVAR = 1: the variants of SURVEY 8(f)-2 switched by the
+// run-time fields of HydroArgs -- a.bulk_one (A26: the bulk moment relaxes with 1, only the deviatoric second-order
+// moments with s_nu) and a.subiter (A27: that many sweeps of the fixed point of eq. 22).
+template <typename T, int Q, int HVAR = 0>
 __device__ __forceinline__ HydroCell<T> hydro_velocity(const Moments<Q, T, true>& m, T c0, T gpx, T gpy, T gpz, T lap, T uox, T uoy,
                                                        T uoz, const HydroArgs<T>& a)
 {
@@ -117,23 +120,39 @@ __device__ __forceinline__ HydroCell<T> hydro_velocity(const Moments<Q, T, true>
 
     // deviatoric second moment without the velocity part
     const T Sxx = m.Pxx - p3, Syy = m.Pyy - p3, Szz = m.Pzz - p3;
-    // viscous force with the velocity of the previous step (eq. 18)
+    // the parts of F that do not depend on u: F_s + F_p (eqs. 14, 16) and F_b (eq. 30)
+    const T F0x = mu * gpx - p3 * grx, F0y = mu * gpy - p3 * gry, F0z = mu * gpz - p3 * grz;
+    const T Fbx = rho * a.gx, Fby = rho * a.gy, Fbz = rho * a.gz;
     const T ts = -tau * s_nu;
-    const T oxx = Sxx - uox * uox, oyy = Syy - uoy * uoy, ozz = Szz - uoz * uoz;
-    const T oxy = m.Pxy - uox * uoy, oxz = m.Pxz - uox * uoz, oyz = m.Pyz - uoy * uoz;
-    const T Fx = mu * gpx - p3 * grx + ts * (oxx * grx + oxy * gry + oxz * grz) + rho * a.gx;
-    const T Fy = mu * gpy - p3 * gry + ts * (oxy * grx + oyy * gry + oyz * grz) + rho * a.gy;
-    const T Fz = mu * gpz - p3 * grz + ts * (oxz * grx + oyz * gry + ozz * grz) + rho * a.gz;
-    // velocity, eq. 22
-    const T hx = T(0.5) * Fx * inv_rho, hy = T(0.5) * Fy * inv_rho, hz = T(0.5) * Fz * inv_rho;
-    const T ux = m.jx + hx, uy = m.jy + hy, uz = m.jz + hz;
+    T hx, hy, hz, ux, uy, uz;
+    const int sweeps = HVAR ? a.subiter : 1;
+    for (int sweep = 0; sweep < sweeps; ++sweep) {
+        // viscous force (eq. 18) with the velocity of the previous step, or of the previous sweep
+        const T oxx = Sxx - uox * uox, oyy = Syy - uoy * uoy, ozz = Szz - uoz * uoz;
+        const T oxy = m.Pxy - uox * uoy, oxz = m.Pxz - uox * uoz, oyz = m.Pyz - uoy * uoz;
+        T Fx = F0x + ts * (oxx * grx + oxy * gry + oxz * grz) + Fbx;
+        T Fy = F0y + ts * (oxy * grx + oyy * gry + oyz * grz) + Fby;
+        T Fz = F0z + ts * (oxz * grx + oyz * gry + ozz * grz) + Fbz;
+        if constexpr (HVAR != 0) {
+            if (a.bulk_one) {
+                // second moment of Omega (g - g^eq) = s_nu Pi_dev + (tr Pi / D) I  instead of s_nu Pi
+                const T tr = Lat<Q>::DIM == 3 ? oxx + oyy + ozz : oxx + oyy;
+                const T tb = -tau * (T(1) - s_nu) * tr * T(1.0 / Lat<Q>::DIM);
+                Fx += tb * grx; Fy += tb * gry; Fz += tb * grz;
+            }
+        }
+        // velocity, eq. 22
+        hx = T(0.5) * Fx * inv_rho; hy = T(0.5) * Fy * inv_rho; hz = T(0.5) * Fz * inv_rho;
+        ux = m.jx + hx; uy = m.jy + hy; uz = m.jz + hz;
+        uox = ux; uoy = uy; uoz = uz;
+    }
     return HydroCell<T>{ux, uy, uz, hx, hy, hz, s_nu, Sxx, Syy, Szz};
 }
 
 // Hydrodynamic collision at one cell (eqs. 10-12, 25 in closed form): emits the
 // post-collision populations through store(ic, value).
-template <typename T, int Q, typename Store>
-__device__ __forceinline__ void hydro_collide(const Moments<Q, T, true>& m, const HydroCell<T>& hc, Store&& store)
+template <typename T, int Q, int HVAR = 0, typename Store>
+__device__ __forceinline__ void hydro_collide(const Moments<Q, T, true>& m, const HydroCell<T>& hc, const HydroArgs<T>& a, Store&& store)
 {
     const T pstar = m.m0;
     const T ux = hc.ux, uy = hc.uy, uz = hc.uz, hx = hc.hx, hy = hc.hy, hz = hc.hz, s_nu = hc.s_nu;
@@ -142,13 +161,22 @@ __device__ __forceinline__ void hydro_collide(const Moments<Q, T, true>& m, cons
     const T om = T(1) - s_nu;
     const T nxx = Sxx - ux * ux, nyy = Syy - uy * uy, nzz = Szz - uz * uz;
     const T k45 = T(4.5) * om, s45 = T(4.5);
-    const T Txx = s45 * ux * ux + k45 * nxx, Tyy = s45 * uy * uy + k45 * nyy, Tzz = s45 * uz * uz + k45 * nzz;
+    T Txx = s45 * ux * ux + k45 * nxx, Tyy = s45 * uy * uy + k45 * nyy, Tzz = s45 * uz * uz + k45 * nzz;
     const T Txy = s45 * ux * uy + k45 * (m.Pxy - ux * uy);
     const T Txz = s45 * ux * uz + k45 * (m.Pxz - ux * uz);
     const T Tyz = s45 * uy * uz + k45 * (m.Pyz - uy * uz);
     // trace of Pi over the lattice's dimensions (D2Q9: the plane only; u_z = 0 there)
     const T trPi = Lat<Q>::DIM == 3 ? nxx + nyy + nzz : nxx + nyy;
-    const T A = pstar - T(1.5) * (ux * ux + uy * uy + uz * uz) - T(1.5) * om * trPi;
+    T A = pstar - T(1.5) * (ux * ux + uy * uy + uz * uz) - T(1.5) * om * trPi;
+    if constexpr (HVAR != 0) {
+        if (a.bulk_one) {
+            // Omega^g = I - (1 - s_nu)(P_2 - P_trace), P_trace x = w_i (|e_i|^2 - D/3) tr Pi(x) / (sum w t^2): Pi becomes trace-free
+            constexpr double inv_norm = Lat<Q>::DIM == 3 ? 1.5 : 2.25;       // 1 / sum_i w_i (|e_i|^2 - D/3)^2
+            const T t = T(inv_norm) * om * trPi;
+            Txx -= t; Tyy -= t; Tzz -= t;
+            A += T(1.5) * om * trPi;
+        }
+    }
     const T bx = T(3) * (ux + hx), by = T(3) * (uy + hy), bz = T(3) * (uz + hz);
     emit_populations<Q, T>(A, bx, by, bz, Txx, Tyy, Tzz, Txy, Txz, Tyz, store);
 }

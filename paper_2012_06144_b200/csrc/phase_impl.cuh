@@ -15,22 +15,9 @@ template <typename T, int Q, bool WALLS, int STATE, int COLL, bool PEER = false>
 __global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const PhaseArgs<T> a)
 {
     int x, y, z;
-#ifdef ACM_PHI_SMEM
-    __shared__ T phi_tile[9 * (ACM_MAXT + 2)];
-    const bool active = cell_of_thread(a.g, x, y, z);
-    const bool tiled = !a.g.linear && blockDim.y == 1 && blockDim.z == 1;      // uniform over the block
-    Nbr nb;
-    if (active) nb.setup<WALLS>(a.g, x, y, z);
-    if (tiled) {
-        if (active) load_phi_tile<T>(phi_tile, a.Csrc, nb, (int)blockDim.x + 2, threadIdx.x == blockDim.x - 1 || x == a.g.nx - 1);
-        __syncthreads();
-    }
-    if (!active) return;
-#else
     if (!cell_of_thread(a.g, x, y, z)) return;
     Nbr nb;
     nb.setup<WALLS>(a.g, x, y, z);
-#endif
     const unsigned idx = nb.at<0, 0, 0>();
     const size_t N = a.N;      // zero-extended 32-bit value
 
@@ -39,10 +26,6 @@ __global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const P
     const T ux = __ldg(a.U + idx), uy = __ldg(a.U + N + idx), uz = __ldg(a.U + 2 * N + idx);
     const T c0 = __ldg(a.Csrc + idx);
     T gx, gy, gz, lap_unused;
-#ifdef ACM_PHI_SMEM
-    if (tiled) fd_phi_acc<Q, T, false>(PhiTile<T>{phi_tile, (int)blockDim.x + 2, (int)threadIdx.x}, c0, gx, gy, gz, lap_unused);
-    else
-#endif
     if constexpr (PEER) fd_phi_peer<Q, T, false>(a.Csrc, nb, a.Cpeer, c0, gx, gy, gz, lap_unused);
     else fd_phi<Q, T, false>(a.Csrc, nb, c0, gx, gy, gz, lap_unused);
 

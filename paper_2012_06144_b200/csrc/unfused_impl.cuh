@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(ACM_MAXT) collide_g_kernel(const HydroArgs<T> 
     m.compute(g);
     HydroCell<T> hc = hydro_velocity<T, Q>(m, c0, gpx, gpy, gpz, lap, uox, uoy, uoz, a);
     hc.ux = Unew[idx]; hc.uy = Unew[N + idx]; hc.uz = Unew[2 * N + idx];
-    hydro_collide<T, Q>(m, hc, [&](auto ic, T v) { st_stream(a.Gdst + (size_t) decltype(ic)::value * N + idx, v); });
+    hydro_collide<T, Q>(m, hc, a, [&](auto ic, T v) { st_stream(a.Gdst + (size_t) decltype(ic)::value * N + idx, v); });
 }
 
 // ---- launchers ------------------------------------------------------------------------------

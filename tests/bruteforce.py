@@ -10,6 +10,11 @@ Gram-Schmidt).  The operators follow from the readings A3/A4 of DESIGN.md:
           (projector on the six second-order moments x^2-1/3, y^2-1/3, z^2-1/3, xy, xz, yz;
            for D2Q9 the last constant is 2/9: three moments x^2-1/3, y^2-1/3, xy)
 
+Variants (A26, A27):
+  bulk_one: the trace moment t_i = |e_i|^2 - D/3 (D = dimension) is taken out of the second-order projector,
+          Omega^g_ij = delta_ij + (s_nu - 1) * [ 9/2 w_i (...) - w_i t_i t_j / sum_k w_k t_k^2 ]
+  subiter: the velocity of eq. 22 by k sweeps of u <- j + F(u)/(2 rho)
+
 Shares nothing with oracle/ or with the CUDA sources; lattices are re-typed here.
 """
 import itertools
@@ -95,7 +100,52 @@ def laplacian(grid, e, w, C, zyx):
     return 6.0 * sum(w[i] * (C[grid.mirror(zyx, e[i], 1)] - C[zyx]) for i in range(1, len(e)))
 
 
-def step(par, H, G, C, U, phase_srt=False):
+def hydro_operator(eg, wg, s, bulk_one=False):
+    """Omega^g(i, j) for the relaxation rate s of the second-order moments (see the module docstring)."""
+    Qg = len(eg)
+    D = 2 if Qg == 9 else 3
+    t = [dot(e, e) - D / 3.0 for e in eg]
+    tnorm = sum(w * v * v for w, v in zip(wg, t))
+
+    def omega_g(i, j):
+        ei, ej = eg[i], eg[j]
+        # (e_i e_i - I/3) : (e_j e_j - I/3) with I the unit tensor of the lattice's dimension (trace 3, or 2 for D2Q9)
+        p2 = dot(ei, ej) ** 2 - dot(ei, ei) / 3.0 - dot(ej, ej) / 3.0 + D / 9.0
+        proj = 4.5 * wg[i] * p2
+        if bulk_one:
+            proj -= wg[i] * t[i] * t[j] / tnorm
+        return (1.0 if i == j else 0.0) + (s - 1.0) * proj
+    return omega_g
+
+
+def hydro_force(par, grid, eg, wg, g, Cn, zyx, u_eq, bulk_one=False):
+    """F = F_s + F_p + F_mu + F_b (eqs. 13-18, 30) at one cell, with g^eq(u_eq) inside F_mu.
+    Returns (F, rho, j = sum g e, gradient of phi)."""
+    Qg = len(eg)
+    beta, kappa = 12.0 * par.sigma / par.xi, 1.5 * par.sigma * par.xi
+    drho = par.rho_H - par.rho_L
+    pstar = sum(g)
+    phi = Cn[zyx]
+    rho = par.rho_L + phi * drho
+    gp = grad(grid, eg, wg, Cn, zyx)
+    lap = laplacian(grid, eg, wg, Cn, zyx)
+    mu = 4.0 * beta * phi * (phi - 1.0) * (phi - 0.5) - kappa * lap
+    gr = [drho * v for v in gp]
+    tau = par.nu_L / CS2 + phi * (par.nu_H / CS2 - par.nu_L / CS2)
+    omega_g = hydro_operator(eg, wg, 1.0 / (tau + 0.5), bulk_one)
+    neq = [g[i] - (pstar * wg[i] + gamma(eg[i], wg[i], u_eq) - wg[i]) for i in range(Qg)]
+    relaxed = [sum(omega_g(i, j) * neq[j] for j in range(Qg)) for i in range(Qg)]
+    Fmu = [0.0, 0.0, 0.0]
+    for a in range(3):
+        for b in range(3):
+            Pi = sum(eg[k][a] * eg[k][b] * relaxed[k] for k in range(Qg))
+            Fmu[a] -= tau * Pi * gr[b]                     # nu/(c_s^2 dt) = tau
+    F = [mu * gp[a] - pstar * CS2 * gr[a] + Fmu[a] + rho * par.gravity[a] for a in range(3)]
+    j = [sum(g[i] * eg[i][a] for i in range(Qg)) for a in range(3)]
+    return F, rho, j, gp
+
+
+def step(par, H, G, C, U, phase_srt=False, bulk_one=False, subiter=1):
     """One coupled step.  phase_srt: Omega^h = omega_phi I (eq. 4 with a single relaxation time).
      H[Qh], G[Qg]: lists of numpy (nz,ny,nx) arrays; C: array; U: list of 3 arrays.
     Returns new (H, G, C, U) in the oracle's storage convention."""
@@ -143,30 +193,12 @@ def step(par, H, G, C, U, phase_srt=False):
         g = [G[i][zyx] for i in range(Qg)]
         pstar = sum(g)
         phi = Cn[zyx]
-        rho = par.rho_L + phi * drho
-        gp = grad(grid, eg, wg, Cn, zyx)
-        lap = laplacian(grid, eg, wg, Cn, zyx)
-        mu = 4.0 * beta * phi * (phi - 1.0) * (phi - 0.5) - kappa * lap
-        gr = [drho * v for v in gp]
         tau = tauL + phi * (tauH - tauL)
-        s = 1.0 / (tau + 0.5)
-
-        def omega_g(i, j):
-            ei, ej = eg[i], eg[j]
-            # (e_i e_i - I/3) : (e_j e_j - I/3) with I the unit tensor of the lattice's dimension (trace 3, or 2 for D2Q9)
-            p2 = dot(ei, ej) ** 2 - dot(ei, ei) / 3.0 - dot(ej, ej) / 3.0 + (2.0 if Qg == 9 else 3.0) / 9.0
-            return (1.0 if i == j else 0.0) + (s - 1.0) * 4.5 * wg[i] * p2
-
-        uo = [U[a][zyx] for a in range(3)]
-        neq = [g[i] - (pstar * wg[i] + gamma(eg[i], wg[i], uo) - wg[i]) for i in range(Qg)]
-        relaxed = [sum(omega_g(i, j) * neq[j] for j in range(Qg)) for i in range(Qg)]
-        Fmu = [0.0, 0.0, 0.0]
-        for a in range(3):
-            for b in range(3):
-                Pi = sum(eg[k][a] * eg[k][b] * relaxed[k] for k in range(Qg))
-                Fmu[a] -= tau * Pi * gr[b]                     # nu/(c_s^2 dt) = tau
-        F = [mu * gp[a] - pstar * CS2 * gr[a] + Fmu[a] + rho * par.gravity[a] for a in range(3)]
-        un = [sum(g[i] * eg[i][a] for i in range(Qg)) + F[a] / (2.0 * rho) for a in range(3)]
+        omega_g = hydro_operator(eg, wg, 1.0 / (tau + 0.5), bulk_one)
+        un = [U[a][zyx] for a in range(3)]
+        for _ in range(subiter):
+            F, rho, j, _ = hydro_force(par, grid, eg, wg, g, Cn, zyx, un, bulk_one)
+            un = [j[a] + F[a] / (2.0 * rho) for a in range(3)]
         Fi = [wg[i] * dot(eg[i], F) / (rho * CS2) for i in range(Qg)]
         d = [pstar * wg[i] + gamma(eg[i], wg[i], un) - wg[i] - g[i] - 0.5 * Fi[i] for i in range(Qg)]
         for i in range(Qg):

@@ -55,7 +55,28 @@ def test_workspace_bytes_and_argument_checks():
     assert lib.acm_step(h, 1) == binding.ACM_ESTATE          # before acm_init
     assert lib.acm_step(h, -1) == binding.ACM_EINVAL
     assert lib.acm_launch_count(h) == 0
+    # a commit without the launches of a full step is refused (Alg. 2's inner / outer order)
+    assert lib.acm_phase_commit(h) == binding.ACM_ESTATE and b"0 of 8" in lib.acm_last_error()
+    assert lib.acm_hydro_commit(h) == binding.ACM_ESTATE
+    assert lib.acm_phase_launch(h, 0, 8) == binding.ACM_ESTATE        # before acm_init
+    # operator variants and CUDA-graph switch: argument checks
+    assert lib.acm_set_subiter(h, 0) == binding.ACM_EINVAL and lib.acm_set_subiter(h, 65) == binding.ACM_EINVAL
+    assert lib.acm_set_subiter(h, 3) == binding.ACM_OK and lib.acm_set_subiter(h, 1) == binding.ACM_OK
+    assert lib.acm_set_graph(h, 2) == binding.ACM_EINVAL and lib.acm_set_graph(h, -1) == binding.ACM_OK
+    assert lib.acm_graph_replays(h) == 0
     lib.acm_destroy(h)
+    h2 = ctypes.c_void_p()
+
+    def create_opt(options):
+        return lib.acm_create_opt(ctypes.byref(h2), 8, 8, 8, 15, 19, 1.0, 1e-3, 1e-4, 5.0, 0.02, 1 / 60, 1 / 60, g, 0, 0, options,
+                                  fake_ws, None)
+    assert create_opt(binding.ACM_OPT_BULK_ONE | binding.ACM_OPT_UNFUSED) == binding.ACM_EINVAL
+    assert create_opt(16) == binding.ACM_EINVAL
+    assert create_opt(binding.ACM_OPT_BULK_ONE | binding.ACM_OPT_INPLACE | binding.ACM_OPT_PHASE_SRT) == binding.ACM_OK
+    lib.acm_destroy(h2)
+    assert create_opt(binding.ACM_OPT_UNFUSED) == binding.ACM_OK
+    assert lib.acm_set_subiter(h2, 2) == binding.ACM_EINVAL           # Algorithm 1 evaluates the forces in two kernels
+    lib.acm_destroy(h2)
 
 
 def test_host_only_bubble_helpers_match_oracle():
