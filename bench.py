@@ -204,6 +204,8 @@ def run_acm(args, rank, local_rank, world):
     phi_h = torch.from_numpy(phi.astype(np_dtype)).pin_memory()
     u_h = torch.from_numpy(u.astype(np_dtype)).pin_memory()
     sim = ACM.from_params(p, precision=precision, device=dev, inplace=args.inplace, unfused=args.unfused)
+    if args.cpt:
+        sim.set_cells_per_thread(args.cpt)
     if args.block:
         sim.set_block(*args.block)
     sim.init(phi_h.to(dev), u_h.to(dev))
@@ -390,6 +392,7 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--block", type=int, nargs=3, default=None)
+    ap.add_argument("--cpt", type=int, default=0, choices=[0, 1, 2], help="cells per thread of the LB kernels (0 = the library's default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--inplace", action="store_true", help="in-place AA streaming (one grid per population set)")
     ap.add_argument("--unfused", action="store_true", help="Algorithm 1 (six kernels per step) as a measured comparison")

@@ -60,6 +60,7 @@ struct acm_ctx {
     int sticky;                 // ACM_OK or ACM_ECUDA
     dim3 block;
     long long launches;
+    int cpt;                    // cells per thread of the two LB kernels: 1, or 2 (pair kernels: 8 / 16-byte accesses, packed fp32)
     int subiter;                // sweeps of the fixed point of eq. 22 (acm_set_subiter; 1 = the single evaluation, A10)
     int phase_planes, hydro_planes;   // owned planes launched since the last acm_*_commit (guard of the split launches)
     // optional per-kernel timing (acm_profile): events recorded around every LB kernel.  The events come from a pool
@@ -125,7 +126,8 @@ static int check_launch(acm_ctx* c, const char* what, cudaError_t e, int count =
 
 // Launch geometry of the two LB kernels: x-rows tiled by the block, or -- when the block is 1-D and
 // nx is not a multiple of it (e.g. the paper's 260^3) -- a linear launch over all cells.
-static bool lb_linear(const acm_ctx* c) { return c->block.y == 1 && c->block.z == 1 && c->nx % (int)c->block.x != 0; }
+// (with two cells per thread a row has nx / 2 pairs)
+static bool lb_linear(const acm_ctx* c) { return c->block.y == 1 && c->block.z == 1 && (c->nx / c->cpt) % (int)c->block.x != 0; }
 
 // geometry block of a launch over the owned planes [z0, z1) (relative to the first owned plane)
 static Geom geom_of(const acm_ctx* c, bool linear, int z0, int z1)
@@ -141,16 +143,17 @@ static Geom geom_of(const acm_ctx* c, bool linear, int z0, int z1)
 }
 static Geom geom_of(const acm_ctx* c) { return geom_of(c, false, 0, c->nzl); }
 
-static Launch launch_over(const acm_ctx* c, dim3 b, bool linear, int nplanes)
+static Launch launch_over(const acm_ctx* c, dim3 b, bool linear, int nplanes, int cpt = 1)
 {
+    const int nxe = c->nx / cpt;      // threads along a row
     if (linear) {
-        const size_t cells = (size_t)c->nx * c->ny * nplanes;
+        const size_t cells = (size_t)nxe * c->ny * nplanes;
         return Launch{dim3((unsigned)((cells + b.x - 1) / b.x), 1, 1), b, c->stream};
     }
-    return Launch{dim3((c->nx + b.x - 1) / b.x, (c->ny + b.y - 1) / b.y, (nplanes + b.z - 1) / b.z), b, c->stream};
+    return Launch{dim3((nxe + b.x - 1) / b.x, (c->ny + b.y - 1) / b.y, (nplanes + b.z - 1) / b.z), b, c->stream};
 }
 
-static Launch lb_launch(const acm_ctx* c, int nplanes) { return launch_over(c, c->block, lb_linear(c), nplanes); }
+static Launch lb_launch(const acm_ctx* c, int nplanes) { return launch_over(c, c->block, lb_linear(c), nplanes, c->cpt); }
 
 template <typename T> static T* wsp(acm_ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }
 
@@ -205,7 +208,8 @@ static int launch_phase_range(acm_ctx* c, int z0, int z1)
     const int coll = (c->options & ACM_OPT_PHASE_SRT) ? PHASE_SRT : PHASE_MRT;
     const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
     cudaError_t e = unfused ? launch_unfused_phase<T>(c->Qh, c->walls != 0, coll, l, a)
-                            : launch_phase<T>(c->Qh, c->walls != 0, c->stH, coll, l, a);
+                    : c->cpt == 2 ? launch_phase2<T>(c->Qh, c->walls != 0, c->stH, coll, l, a)
+                                  : launch_phase<T>(c->Qh, c->walls != 0, c->stH, coll, l, a);
     c->phase_planes += z1 - z0;
     return check_launch(c, unfused ? "stream_h/phi/collide_h kernels" : "phase_kernel", e, unfused ? 3 : 1);
 }
@@ -240,7 +244,8 @@ static int launch_hydro_range(acm_ctx* c, int z0, int z1)
     const Launch l = lb_launch(c, z1 - z0);
     const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
     cudaError_t e = unfused ? launch_unfused_hydro<T>(c->Qg, c->walls != 0, l, a, wsp<T>(c, c->offU[c->curU]), wsp<T>(c, c->offU[c->curU ^ 1]))
-                            : launch_hydro<T>(c->Qg, c->walls != 0, c->stG, l, a);
+                    : c->cpt == 2 ? launch_hydro2<T>(c->Qg, c->walls != 0, c->stG, l, a)
+                                  : launch_hydro<T>(c->Qg, c->walls != 0, c->stG, l, a);
     c->hydro_planes += z1 - z0;
     return check_launch(c, unfused ? "stream_g/velocity/collide_g kernels" : "hydro_kernel", e, unfused ? 3 : 1);
 }
@@ -486,9 +491,12 @@ static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase,
     c->stH = c->stG = ST_POST;
     c->initialised = false;
     c->sticky = ACM_OK;
+    // fp32: two cells per thread (8-byte accesses, packed fp32 arithmetic) whenever the rows allow it; fp64: one
+    // (the 16-byte pairing is a measured wash; acm_set_cells_per_thread switches either)
+    c->cpt = (precision == ACM_F32 && nx % 2 == 0 && !(options & ACM_OPT_UNFUSED)) ? 2 : 1;
     // one block = 1 KB of every population row (measured best on B200 for both precisions, profiles/): 128 fp64
-    // or 256 fp32 cells along x; fp32 falls back to 128 when nx is not a multiple of 256
-    c->block = (precision == ACM_F32 && nx % 256 == 0) ? dim3(256, 1, 1) : dim3(128, 1, 1);
+    // cells or 256 fp32 cells (128 pairs) along x; single-cell fp32 falls back to 128 when nx is not a multiple of 256
+    c->block = (precision == ACM_F32 && c->cpt == 1 && nx % 256 == 0) ? dim3(256, 1, 1) : dim3(128, 1, 1);
     c->launches = 0;
     c->subiter = 1;
     c->phase_planes = c->hydro_planes = 0;
@@ -727,6 +735,18 @@ int acm_set_block(acm_ctx* c, int bx, int by, int bz)
         return fail(ACM_EINVAL, "acm_set_block: need 1 <= bx*by*bz <= 256");
     if (c->phase_planes || c->hydro_planes) return fail(ACM_ESTATE, "acm_set_block: a step is partly launched (commit it first)");
     c->block = dim3(bx, by, bz);
+    graphs_clear(c);
+    return ACM_OK;
+}
+
+int acm_set_cells_per_thread(acm_ctx* c, int n)
+{
+    ACM_CHECK_CTX(c);
+    if (n != 1 && n != 2) return fail(ACM_EINVAL, "acm_set_cells_per_thread: 1 or 2");
+    if (n == 2 && (c->nx % 2 != 0 || (c->options & ACM_OPT_UNFUSED)))
+        return fail(ACM_EINVAL, "acm_set_cells_per_thread: two cells per thread need an even nx and the fused kernels");
+    if (c->phase_planes || c->hydro_planes) return fail(ACM_ESTATE, "acm_set_cells_per_thread: a step is partly launched (commit it first)");
+    c->cpt = n;
     graphs_clear(c);
     return ACM_OK;
 }

@@ -18,6 +18,11 @@ template <typename T> cudaError_t launch_phase(int Q, bool walls, int state, int
 // Fused hydrodynamic LB step (one launch).
 template <typename T> cudaError_t launch_hydro(int Q, bool walls, int state, const Launch& l, const HydroArgs<T>& a);
 
+// The same two kernels with two x-adjacent cells per thread (pair.cuh): l.block.x threads cover 2 l.block.x cells
+// of a row; needs nx even.
+template <typename T> cudaError_t launch_phase2(int Q, bool walls, int state, int collision, const Launch& l, const PhaseArgs<T>& a);
+template <typename T> cudaError_t launch_hydro2(int Q, bool walls, int state, const Launch& l, const HydroArgs<T>& a);
+
 // Algorithm 1, three launches each: stream h -> update phi -> collide h, and
 // stream g -> update u (Uold -> Unew) -> collide g.  Two-grid storage only (a.Hsrc/a.Gsrc in ST_POST).
 template <typename T> cudaError_t launch_unfused_phase(int Q, bool walls, int collision, const Launch& l, const PhaseArgs<T>& a);

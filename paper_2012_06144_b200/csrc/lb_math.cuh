@@ -3,6 +3,7 @@
 // (unfused_impl.cuh: Algorithm 1), so that both evaluate exactly the same expressions.
 #pragma once
 #include "common.cuh"
+#include "vec2.cuh"
 
 namespace acm {
 
@@ -15,12 +16,12 @@ __device__ __forceinline__ void phase_collide(const T (&h)[Q], const Moments<Q, 
 {
     // fp32 instance (A22): h and phi are stored as deviations from the reference phase `ref` (0 or 1),
     // h_i - ref w_i and phi - ref, so that the bulk of that phase keeps its digits; fp64: ref = 0, nothing changes
-    constexpr bool DEV = sizeof(T) == 4;
+    constexpr bool DEV = is_f32<T>;
     const T phid = m.m0;                             // stored zeroth moment
     const T phi = DEV ? ref + phid : phid;           // the order parameter itself
     // interface normal (n = 0 where grad phi vanishes exactly) and theta = (1 - 4 (phi-1/2)^2)/xi
     const T g2 = gx * gx + gy * gy + gz * gz;
-    const T inv = (g2 > T(0)) ? T(1) / sqrt(g2) : T(0);
+    const T inv = inv_norm_or_zero(g2);
     T theta;
     if constexpr (DEV) {
         theta = T(4) * (ref + c0) * ((T(1) - ref) - c0) * inv_xi;     // 1 - 4 (phi - 1/2)^2 = 4 phi (1 - phi), c0 = phi_old - ref
@@ -65,7 +66,7 @@ __device__ __forceinline__ void phase_collide(const T (&h)[Q], const Moments<Q, 
         if constexpr (COLL == PHASE_SRT) return v + keep * h[decltype(ic)::value];
         else return v;
     };
-    if constexpr (sizeof(T) == 8) {
+    if constexpr (!DEV) {
         emit_populations<Q, T>(A, bx, by, bz, Ts * ux * ux, Ts * uy * uy, Ts * uz * uz, Ts * ux * uy, Ts * ux * uz,
                                Ts * uy * uz, [&](auto ic, T v) {
                                    store(ic, post(ic, v));
@@ -102,9 +103,10 @@ struct HydroCell {
 // HVAR = 0: the default operators (readings A4, A10).  HVAR = 1: the variants of SURVEY 8(f)-2 switched by the
 // run-time fields of HydroArgs -- a.bulk_one (A26: the bulk moment relaxes with 1, only the deviatoric second-order
 // moments with s_nu) and a.subiter (A27: that many sweeps of the fixed point of eq. 22).
-template <typename T, int Q, int HVAR = 0>
+// T is the element type the arithmetic runs in (a cell, or a pair of cells: vec2.cuh), S the scalar type of the arguments.
+template <typename T, int Q, int HVAR = 0, typename S>
 __device__ __forceinline__ HydroCell<T> hydro_velocity(const Moments<Q, T, true>& m, T c0, T gpx, T gpy, T gpz, T lap, T uox, T uoy,
-                                                       T uoz, const HydroArgs<T>& a)
+                                                       T uoz, const HydroArgs<S>& a)
 {
     const T pstar = m.m0;
     const T p3 = pstar * T(1.0 / 3.0);
@@ -114,8 +116,9 @@ __device__ __forceinline__ HydroCell<T> hydro_velocity(const Moments<Q, T, true>
     const T inv_rho = T(1) / rho;
     const T tau = a.tau_L + c0 * a.dtau;                  // eq. 20
     const T s_nu = T(1) / (tau + T(0.5));                 // eq. 21
-    const T mu = (sizeof(T) == 4 ? a.beta4 * (a.ref + c0) * (c0 - (T(1) - a.ref)) * (c0 + (a.ref - T(0.5)))
-                                 : a.beta4 * c0 * (c0 - T(1)) * (c0 - T(0.5))) - a.kappa * lap;   // eq. 17
+    T mu;                                                 // eq. 17
+    if constexpr (is_f32<T>) mu = a.beta4 * (a.ref + c0) * (c0 - (T(1) - a.ref)) * (c0 + (a.ref - T(0.5))) - a.kappa * lap;
+    else mu = a.beta4 * c0 * (c0 - T(1)) * (c0 - T(0.5)) - a.kappa * lap;
     const T grx = a.drho * gpx, gry = a.drho * gpy, grz = a.drho * gpz;
 
     // deviatoric second moment without the velocity part
@@ -151,8 +154,8 @@ __device__ __forceinline__ HydroCell<T> hydro_velocity(const Moments<Q, T, true>
 
 // Hydrodynamic collision at one cell (eqs. 10-12, 25 in closed form): emits the
 // post-collision populations through store(ic, value).
-template <typename T, int Q, int HVAR = 0, typename Store>
-__device__ __forceinline__ void hydro_collide(const Moments<Q, T, true>& m, const HydroCell<T>& hc, const HydroArgs<T>& a, Store&& store)
+template <typename T, int Q, int HVAR = 0, typename S, typename Store>
+__device__ __forceinline__ void hydro_collide(const Moments<Q, T, true>& m, const HydroCell<T>& hc, const HydroArgs<S>& a, Store&& store)
 {
     const T pstar = m.m0;
     const T ux = hc.ux, uy = hc.uy, uz = hc.uz, hx = hc.hx, hy = hc.hy, hz = hc.hz, s_nu = hc.s_nu;
