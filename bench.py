@@ -120,37 +120,68 @@ class ClockSampler:
                 "reasons": sorted(self.reasons), "samples": len(s)}
 
 
-def oracle_sample(config, budget_s, steps=None):
+def oracle_sample(config, budget_s, steps=None, threads=0):
     """Times the oracle as it stands on the host cores, on a bounded sample of the workload:
     the same recipe on a smaller cube.  Returns (mlups, cores, description, steps, seconds)."""
     from oracle import Oracle, oracle as om
+    all_cores = om.set_threads(0)
+    cores = om.set_threads(threads) if threads else all_cores
+    try:
+        # calibrate on 24^3
+        base = config if config in (1, 3, 5, 6, 7) else 3
+        sz = (lambda n: int(round(n ** 1.5))) if base == 7 else (lambda n: n)      # 2-D: the same number of cells as n^3
+        p, phi, u, _ = workload(base, size=sz(24))
+        o = Oracle.from_params(p)
+        o.init(phi, u)
+        o.step(1)
+        t = time.perf_counter()
+        o.step(2)
+        per_cell = (time.perf_counter() - t) / (2 * p.ncells)
+        del o
+        if steps is None:
+            n, steps = 64, max(2, min(20, int(budget_s / (per_cell * 64 ** 3))))
+            while n > 24 and per_cell * n ** 3 * steps > 1.5 * budget_s:
+                n -= 8
+        else:
+            n = 64
+            while n > 16 and per_cell * n ** 3 * steps > budget_s:
+                n -= 8
+        p, phi, u, name = workload(base, size=sz(n))
+        o = Oracle.from_params(p)
+        o.init(phi, u)
+        t = time.perf_counter()
+        o.step(steps)
+        dt = time.perf_counter() - t
+    finally:
+        om.set_threads(all_cores)
+    return p.ncells * steps / dt / 1e6, cores, f"{name} ({steps} steps; same recipe as the benchmark workload)", steps, dt
+
+
+def oracle_full_size(config, p, phi, u, steps=3, max_cells=1 << 24):
+    """The oracle on the REAL input of the workload for a few steps (256^3 x 3 steps), all cores."""
+    if p.ncells > max_cells:
+        return None
+    from oracle import Oracle, oracle as om
     cores = om.set_threads(0)
-    # calibrate on 24^3
-    base = config if config in (1, 3, 5, 6, 7) else 3
-    sz = (lambda n: int(round(n ** 1.5))) if base == 7 else (lambda n: n)      # 2-D: the same number of cells as n^3
-    p, phi, u, _ = workload(base, size=sz(24))
-    o = Oracle.from_params(p)
-    o.init(phi, u)
-    o.step(1)
-    t = time.perf_counter()
-    o.step(2)
-    per_cell = (time.perf_counter() - t) / (2 * p.ncells)
-    del o
-    if steps is None:
-        n, steps = 64, max(2, min(20, int(budget_s / (per_cell * 64 ** 3))))
-        while n > 24 and per_cell * n ** 3 * steps > 1.5 * budget_s:
-            n -= 8
-    else:
-        n = 64
-        while n > 16 and per_cell * n ** 3 * steps > budget_s:
-            n -= 8
-    p, phi, u, name = workload(base, size=sz(n))
     o = Oracle.from_params(p)
     o.init(phi, u)
     t = time.perf_counter()
     o.step(steps)
     dt = time.perf_counter() - t
-    return p.ncells * steps / dt / 1e6, cores, f"{name} ({steps} steps; same recipe as the benchmark workload)", steps, dt
+    return {"value": p.ncells * steps / dt / 1e6, "unit": UNIT, "cores": cores, "steps": steps, "seconds": dt,
+            "sample": f"the benchmark input itself, {p.nx}x{p.ny}x{p.nz}, {steps} steps"}
+
+
+def cpu_baseline(config, p, phi, u):
+    """cpu_baseline object: the oracle as it stands on the box's host cores (reported, not a target)."""
+    v, cores, sample, _, _ = oracle_sample(config, budget_s=10.0)
+    out = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+    v1, c1, s1, _, dt1 = oracle_sample(config, budget_s=4.0, threads=1)
+    out["single_thread"] = {"value": v1, "unit": UNIT, "cores": c1, "seconds": dt1, "sample": s1}
+    full = oracle_full_size(config, p, phi, u)
+    if full is not None:
+        out["full_size"] = full
+    return out
 
 
 def run_reference(args, rank, world):
@@ -182,23 +213,32 @@ def workload_name_only(config):
     return None, None, None, names[config]
 
 
-def run_acm(args, rank, local_rank, world):
+NOMINAL_HBM_GBS = 8000.0      # vendor figure for context (B200_PROFILING.md: 7.7 TB/s HGX, 8 TB/s DGX)
+REPEATS = 5
+
+
+def traffic_row(kernel, config, precision):
+    """DRAM bytes per launch of that kernel from the committed ncu --set full capture (profiles/traffic.csv) and the
+    commit of the build it was captured from."""
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
+    if os.path.exists(tpath):
+        import csv
+        for row in csv.DictReader(open(tpath)):
+            if (row["kernel"], row["config"], row["precision"]) == (kernel, str(config), precision):
+                return float(row["dram_bytes_per_launch"]), row.get("commit") or None
+    return None, None
+
+
+def measure(args, config, precision, dev, local_rank, world, K, W, with_e2e=True):
+    """Device-resident throughput of one workload: W warm-up steps, then REPEATS back-to-back intervals of exactly K
+    steps each (no per-kernel instrumentation inside them), each bracketed by CUDA events on the launching stream,
+    max over ranks per interval, median over the intervals; then a separate pass of K steps with per-kernel events
+    (acm_profile) for the kernel split; then the end-to-end run through acm_run_host."""
     import torch
     from paper_2012_06144_b200 import replicas
     from paper_2012_06144_b200.binding import ACM
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    replicas.init("nccl", dev)
-
-    def barrier():
-        replicas.barrier(dev)
-
-    K, W = args.steps, max(args.warmup, 3)
-    p, phi, u, name = workload(args.config)
-    precision = args.precision
+    p, phi, u, name = workload(config)
     esz = 8 if precision == "f64" else 4
     np_dtype = "float64" if precision == "f64" else "float32"
     phi_h = torch.from_numpy(phi.astype(np_dtype)).pin_memory()
@@ -212,84 +252,125 @@ def run_acm(args, rank, local_rank, world):
     N = p.ncells
     b_phase, b_hydro = bytes_per_cell(p.stencil_phase, p.stencil_hydro, esz)
 
-    # ---- device-resident throughput: W warm-up steps, then exactly K timed steps ----
     sim.step(W)
-    barrier()
+    replicas.barrier(dev)
     launches0 = sim.launch_count
-    sim.profile(True)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(REPEATS + 1)]
     with ClockSampler(local_rank) as clk:
-        e0.record()
-        sim.step(K)
-        e1.record()
-        barrier()
-    ms = e0.elapsed_time(e1)
-    phase_ms, hydro_ms, nprof = sim.profile_read()
-    sim.profile(False)
-    launches = sim.launch_count - launches0
-    mass = sim.phi_mass()
-    ms = replicas.max_over_ranks(ms, dev)
+        ev[0].record()
+        for r in range(REPEATS):
+            sim.step(K)
+            ev[r + 1].record()
+        replicas.barrier(dev)
+    launches = (sim.launch_count - launches0) // REPEATS
+    intervals = sorted(replicas.max_over_ranks(ev[r].elapsed_time(ev[r + 1]), dev) for r in range(REPEATS))
+    ms = intervals[REPEATS // 2]
     value = replicas.aggregate_mlups(N, K, ms, world)
 
-    # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region ----
-    po, uo, pro = (torch.empty_like(phi_h).pin_memory(), torch.empty_like(u_h).pin_memory(),
-                   torch.empty_like(phi_h).pin_memory())
-    Ke = K
-    sim.run_host(phi_h, u_h, 2, po, uo, pro)            # warm the path
-    barrier()
-    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t0.record()
-    sim.run_host(phi_h, u_h, Ke, po, uo, pro)
-    t1.record()
-    barrier()
-    ms_e2e = t0.elapsed_time(t1)
-    ms_e2e = replicas.max_over_ranks(ms_e2e, dev)
-    e2e = replicas.aggregate_mlups(N, Ke, ms_e2e, world)
-    finite = bool(torch.isfinite(po).all() and torch.isfinite(uo).all())
+    # per-kernel split: a separate, instrumented pass (events from a pool created before the first kernel)
+    sim.profile(True)
+    sim.step(K)
+    phase_ms, hydro_ms, nprof = sim.profile_read()
+    sim.profile(False)
+    phase_ms, hydro_ms = phase_ms / max(nprof, 1), hydro_ms / max(nprof, 1)
+    mass = sim.phi_mass()
+
+    res = {"p": p, "phi": phi, "u": u, "name": name, "N": N, "esz": esz, "value": value, "ms": ms, "intervals": intervals,
+           "value_min": replicas.aggregate_mlups(N, K, intervals[-1], world), "value_max": replicas.aggregate_mlups(N, K, intervals[0], world),
+           "phase_ms": phase_ms, "hydro_ms": hydro_ms, "launches": launches, "mass": mass, "clocks": clk.summary(),
+           "b_phase": b_phase, "b_hydro": b_hydro}
+
+    if with_e2e:
+        # end to end through the C ABI with host buffers (pinned), copies inside the timed region
+        po, uo, pro = (torch.empty_like(phi_h).pin_memory(), torch.empty_like(u_h).pin_memory(), torch.empty_like(phi_h).pin_memory())
+        sim.run_host(phi_h, u_h, 2, po, uo, pro)            # warm the path
+        replicas.barrier(dev)
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0.record()
+        sim.run_host(phi_h, u_h, K, po, uo, pro)
+        t1.record()
+        replicas.barrier(dev)
+        ms_e2e = replicas.max_over_ranks(t0.elapsed_time(t1), dev)
+        res["e2e"] = replicas.aggregate_mlups(N, K, ms_e2e, world)
+        res["finite"] = bool(torch.isfinite(po).all() and torch.isfinite(uo).all())
+    del sim
+    torch.cuda.empty_cache()
+    return res
+
+
+def roofline_of(args, config, precision, r, K):
+    peak, peak_src = measured_peaks()
+    dom = "hydro_kernel" if r["hydro_ms"] >= r["phase_ms"] else "phase_kernel"     # unfused: the three kernels of that LB step
+    dom_ms = r["hydro_ms"] if dom == "hydro_kernel" else r["phase_ms"]
+    dom_bytes = (r["b_hydro"] if dom == "hydro_kernel" else r["b_phase"]) * r["N"]
+    achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
+    step_gbs = (r["b_phase"] + r["b_hydro"]) * r["N"] * K / (r["ms"] * 1e-3) / 1e9
+    traffic, commit = traffic_row(dom, config, precision)
+    roof = {"bound": "hbm", "kernel": dom if not args.unfused else
+            dom.replace("_kernel", "") + " step as three kernels (stream, update, collide); bytes = the fused kernel's algorithmic count",
+            "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "traffic_commit": commit,
+            "peak_source": peak_src + " -- a plain copy: a lower bound of what HBM delivers, fractions above 1 are possible",
+            "peak_is_lower_bound": achieved > peak, "frac_of_nominal": achieved / NOMINAL_HBM_GBS, "peak_nominal": NOMINAL_HBM_GBS,
+            "algorithmic_bytes_per_launch": dom_bytes, "kernel_ms": dom_ms,
+            "kernel_share_of_step": dom_ms / (r["phase_ms"] + r["hydro_ms"])}
+    return roof, step_gbs, peak
+
+
+def run_acm(args, rank, local_rank, world):
+    import torch
+    from paper_2012_06144_b200 import replicas
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    replicas.init("nccl", dev)
+
+    K, W = args.steps, max(args.warmup, 20)      # never fewer than 20 warm-up steps
+    precision = args.precision
+    r = measure(args, args.config, precision, dev, local_rank, world, K, W)
+    extras = []
+    if args.config == 3 and precision == "f64" and world == 1 and not (args.no_extras or args.inplace or args.unfused or args.cpt or args.block):
+        # the fp32 instance of config 5 (BASELINE.json configs[4]) in the same run: device-resident throughput only
+        x = measure(args, 5, "f32", dev, local_rank, world, K, W, with_e2e=False)
+        roof, step_gbs, peak = roofline_of(args, 5, "f32", x, K)
+        extras.append({"workload": x["name"], "dtype": "f32", "value": x["value"], "value_min": x["value_min"], "value_max": x["value_max"],
+                       "unit": UNIT, "ms_per_step": x["ms"] / K, "phase_ms": x["phase_ms"], "hydro_ms": x["hydro_ms"],
+                       "bytes_per_cell": {"phase": x["b_phase"], "hydro": x["b_hydro"]}, "step_algorithmic_GBps": step_gbs,
+                       "step_frac_of_peak": step_gbs / peak, "roofline": roof})
 
     if rank == 0:
-        peak, peak_src = measured_peaks()
-        # dominant kernel = the one with the larger share of the step
-        dom = "hydro_kernel" if hydro_ms >= phase_ms else "phase_kernel"     # unfused: the three kernels of that LB step
-        dom_ms = (hydro_ms if dom == "hydro_kernel" else phase_ms) / max(nprof, 1)
-        dom_bytes = (b_hydro if dom == "hydro_kernel" else b_phase) * N
-        achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
-        step_gbs = (b_phase + b_hydro) * N * K / (ms * 1e-3) / 1e9
-        traffic = None      # DRAM bytes per launch of that kernel from the committed ncu --set full capture
-        tpath = os.path.join(ROOT, "profiles", "traffic.csv")
-        if os.path.exists(tpath):
-            import csv
-            for row in csv.DictReader(open(tpath)):
-                if (row["kernel"], row["config"], row["precision"]) == (dom, str(args.config), precision):
-                    traffic = float(row["dram_bytes_per_launch"])
+        p, N, esz, ms = r["p"], r["N"], r["esz"], r["ms"]
+        roof, step_gbs, peak = roofline_of(args, args.config, precision, r, K)
         out = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+            "metric": METRIC, "value": r["value"], "value_min": r["value_min"], "value_max": r["value_max"], "unit": UNIT, "n_gpus": world,
+            "steps": K, "warmup": W, "repeats": REPEATS, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
             # BASELINE.md holds the paper's number only for its own benchmark (config 6: 550 MLUPS, P100)
-            "vs_baseline": (value / (211.0 if args.unfused else 550.0) if args.config == 6 and world == 1 and precision == "f64" else None),
+            "vs_baseline": (r["value"] / (211.0 if args.unfused else 550.0) if args.config == 6 and world == 1 and precision == "f64" else None),
             "dtype": precision, "data": "synthetic",
-            "config": {"workload": name, "grid": [p.nx, p.ny, p.nz], "stencils": [p.stencil_phase, p.stencil_hydro], "phase_collision": "SRT" if p.phase_srt else "MRT", "streaming": "in-place AA" if args.inplace else "two-grid pull",
+            "config": {"workload": r["name"], "grid": [p.nx, p.ny, p.nz], "stencils": [p.stencil_phase, p.stencil_hydro], "phase_collision": "SRT" if p.phase_srt else "MRT", "streaming": "in-place AA" if args.inplace else "two-grid pull",
                        "algorithm": "Algorithm 1: six unfused kernels (comparison)" if args.unfused else "Algorithm 2: two fused kernels",
                        "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "timing": f"median of {REPEATS} back-to-back intervals of {K} steps (CUDA events, no per-kernel instrumentation inside); "
+                                 f"value_min / value_max = slowest / fastest interval; kernel split from a separate instrumented pass",
+                       "interval_ms": r["intervals"],
                        "l2": f"inputs larger than L2: {(2 * (p.stencil_phase + p.stencil_hydro) + 5) * N * esz / 1e9:.1f} GB "
                              "of state streamed every step vs 126 MB L2",
-                       "bytes_per_cell": {"phase": b_phase, "hydro": b_hydro},
-                       "step_algorithmic_GBps": step_gbs, "step_frac_of_peak": step_gbs / peak,
-                       "phase_ms": phase_ms / max(nprof, 1), "hydro_ms": hydro_ms / max(nprof, 1),
-                       "sum_phi": mass, "finite": finite},
-            "clocks": clk.summary(),
-            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 4 * N * esz / Ke,
-                    "d2h_bytes_per_step": 5 * N * esz / Ke, "steps": Ke,
+                       "bytes_per_cell": {"phase": r["b_phase"], "hydro": r["b_hydro"]},
+                       "step_algorithmic_GBps": step_gbs, "step_frac_of_peak": step_gbs / peak, "step_frac_of_nominal": step_gbs / NOMINAL_HBM_GBS,
+                       "phase_ms": r["phase_ms"], "hydro_ms": r["hydro_ms"],
+                       "sum_phi": r["mass"], "finite": r["finite"]},
+            "clocks": r["clocks"],
+            "e2e": {"value": r["e2e"], "unit": UNIT, "h2d_bytes_per_step": 4 * N * esz / K,
+                    "d2h_bytes_per_step": 5 * N * esz / K, "steps": K,
                     "what": "acm_run_host: pinned host phi,u -> device, init, K steps, fields, phi,u,p -> host"},
-            "gpu_launches": launches,
-            "roofline": {"bound": "hbm", "kernel": dom if not args.unfused else
-                         dom.replace("_kernel", "") + " step as three kernels (stream, update, collide); bytes = the fused kernel's algorithmic count", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": dom_bytes, "kernel_ms": dom_ms},
+            "gpu_launches": r["launches"],
+            "roofline": roof,
         }
+        if extras:
+            out["also"] = extras
         if not args.no_cpu_baseline and world == 1:
-            v, cores, sample, _, _ = oracle_sample(args.config, budget_s=15.0)
-            out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+            out["cpu_baseline"] = cpu_baseline(args.config, p, r["phi"], r["u"])
         print(json.dumps(out), flush=True)
     replicas.shutdown()
 
@@ -308,7 +389,7 @@ def run_decomposed(args, rank, local_rank, world):
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     replicas.init("nccl", dev)
-    K, W = args.steps, max(args.warmup, 3)
+    K, W = args.steps, max(args.warmup, 20)
     p, phi, u, name = workload(args.config)
     if p.wall_flags & 4:
         raise SystemExit("--decompose stacks the workload along z: it must be periodic in z")
@@ -345,6 +426,19 @@ def run_decomposed(args, rank, local_rank, world):
     N = p.ncells
     value = replicas.aggregate_mlups(N, K, ms, world)
     mass = slab.phi_mass()
+    # evidence that every rank drove its own GPU and, in peer mode, that the neighbours' memory is reachable
+    # (NCCL_DEBUG is left as the caller set it: NCCL_DEBUG=INFO shows the communicator and the transports)
+    import torch.distributed as dist
+    props = torch.cuda.get_device_properties(dev)
+    nbrs = sorted({(rank - 1) % world, (rank + 1) % world} - {rank})
+    mine = {"rank": rank, "device": local_rank, "name": props.name, "uuid": str(getattr(props, "uuid", "")),
+            "launches": launches, "peak_alloc_GB": torch.cuda.max_memory_allocated(dev) / 1e9,
+            "peer_access": {str(n): bool(torch.cuda.can_device_access_peer(local_rank, n % torch.cuda.device_count()))
+                            for n in nbrs if n % torch.cuda.device_count() != local_rank}}
+    ranks_info = [mine]
+    if world > 1:
+        ranks_info = [None] * world
+        dist.all_gather_object(ranks_info, mine)
     # end to end: host -> device, init, halos, K steps, fields -> host
     po, uo = torch.empty_like(phi_h).pin_memory(), torch.empty_like(u_h).pin_memory()
     replicas.barrier(dev)
@@ -361,7 +455,7 @@ def run_decomposed(args, rank, local_rank, world):
     if rank == 0:
         peak, peak_src = measured_peaks()
         b_phase, b_hydro = bytes_per_cell(p.stencil_phase, p.stencil_hydro, esz)
-        step_gbs = (b_phase + b_hydro) * N * K / (ms * 1e-3) / 1e9
+        step_gbs = (b_phase + b_hydro) * N * K / (ms * 1e-3) / 1e9      # N = cells of ONE rank: already the per-GPU rate
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": precision, "data": "synthetic",
                "config": {"workload": name + f", stacked {world}x along z and decomposed into {world} z-slabs",
@@ -370,14 +464,17 @@ def run_decomposed(args, rank, local_rank, world):
                                          ("peer mode: kernels read the neighbours' planes directly, one signal per kernel" if args.peer else
                                           "halo exchange " + ("overlapped on a second stream" if run.comm is not None else "in stream order")),
                           "l2": "inputs larger than L2 (per rank as in the single-GPU run)",
-                          "bytes_per_cell": {"phase": b_phase, "hydro": b_hydro}, "sum_phi_rank0": mass},
+                          "bytes_per_cell": {"phase": b_phase, "hydro": b_hydro}, "sum_phi_rank0": mass,
+                          "ranks": ranks_info, "gpus_active": len({r["uuid"] or r["device"] for r in ranks_info}),
+                          "nccl": {"version": ".".join(str(v) for v in torch.cuda.nccl.version()) if world > 1 else None,
+                                   "NCCL_DEBUG": os.environ.get("NCCL_DEBUG")}},
                "clocks": clk.summary(),
                "e2e": {"value": replicas.aggregate_mlups(N, K, ms_e2e, world), "unit": UNIT, "h2d_bytes_per_step": 4 * N * esz / K,
                        "d2h_bytes_per_step": 4 * N * esz / K, "steps": K,
                        "what": "per rank: pinned host phi,u -> device, init, halo exchange, K steps, phi,u -> host"},
                "gpu_launches": launches,
                "roofline": {"bound": "hbm", "kernel": "phase + hydro kernels of one rank (whole step, slab schedule)",
-                            "achieved": step_gbs / world, "peak": peak, "unit": "GB/s", "frac": step_gbs / world / peak,
+                            "achieved": step_gbs, "peak": peak, "unit": "GB/s", "frac": step_gbs / peak, "frac_of_nominal": step_gbs / NOMINAL_HBM_GBS,
                             "traffic": None, "peak_source": peak_src}}
         print(json.dumps(out), flush=True)
     replicas.shutdown()
@@ -394,6 +491,7 @@ def main():
     ap.add_argument("--block", type=int, nargs=3, default=None)
     ap.add_argument("--cpt", type=int, default=0, choices=[0, 1, 2], help="cells per thread of the LB kernels (0 = the library's default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the extra fp32 config-5 measurement of the default run")
     ap.add_argument("--inplace", action="store_true", help="in-place AA streaming (one grid per population set)")
     ap.add_argument("--unfused", action="store_true", help="Algorithm 1 (six kernels per step) as a measured comparison")
     ap.add_argument("--decompose", action="store_true", help="one global domain in z-slabs with halo exchange instead of replicas")

@@ -245,6 +245,13 @@ int acm_halo_plan(const acm_ctx*, int what, int side, int recv, int max_chunks, 
  * Both NULL switches peer mode off.  acm_get_pdfs / acm_fields(p) still read ghost planes: refresh them first. */
 int acm_set_peers(acm_ctx*, void* lo_workspace, void* hi_workspace);
 
+/* What must agree between the slabs of a decomposition in PEER mode, because a slab addresses its neighbours' arrays
+ * with its OWN offsets and buffer parity: out = { workspace bytes of the layout, byte offsets of the current h, g and
+ * phi buffers, hydrodynamic steps committed since acm_init, owned planes, 1 if a step is partly launched,
+ * fp32 reference phase (0: fp64, 1: light, 2: heavy) }.  Host only.  The caller compares the tuples of all ranks
+ * (slab.py does at set-up, after init and before it reads neighbour memory for the exports). */
+int acm_state_signature(const acm_ctx*, unsigned long long out[8]);
+
 /* Launch one LB kernel on the owned planes [z0, z1) (0 <= z0 <= z1 <= owned planes; empty range = no launch)
  * without flipping the buffers; the *_commit call flips them once all planes of the step are launched.
  * Also valid on a plain context, where acm_step(1) equals launch(0, nz), commit for both kernels.

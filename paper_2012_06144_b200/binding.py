@@ -19,7 +19,7 @@ ACM_OPT_INPLACE, ACM_OPT_PHASE_SRT, ACM_OPT_UNFUSED, ACM_OPT_BULK_ONE = 1, 2, 4,
 
 EXPORTS = ["acm_workspace_bytes", "acm_workspace_bytes_opt", "acm_create", "acm_create_opt", "acm_init", "acm_step", "acm_fields", "acm_phi_mass", "acm_get_pdfs",
            "acm_set_pdfs", "acm_run_host", "acm_set_reference_phase", "acm_bubble_diag", "acm_bubble_sums", "acm_slab_range", "acm_workspace_bytes_slab", "acm_create_slab", "acm_slab_info",
-           "acm_halo_plan", "acm_set_peers", "acm_phase_launch", "acm_phase_commit", "acm_hydro_launch", "acm_hydro_commit", "acm_bubble_params", "acm_drag_lbm", "acm_drag_exp", "acm_set_block", "acm_set_cells_per_thread", "acm_set_subiter", "acm_set_graph", "acm_graph_replays", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
+           "acm_halo_plan", "acm_set_peers", "acm_state_signature", "acm_phase_launch", "acm_phase_commit", "acm_hydro_launch", "acm_hydro_commit", "acm_bubble_params", "acm_drag_lbm", "acm_drag_exp", "acm_set_block", "acm_set_cells_per_thread", "acm_set_subiter", "acm_set_graph", "acm_graph_replays", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
 
 _lib = None
 
@@ -70,6 +70,7 @@ def load(build_if_missing: bool = True):
     lib.acm_slab_info.argtypes = [vp, C.POINTER(i32)]
     lib.acm_halo_plan.argtypes = [vp, i32, i32, i32, i32, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
     lib.acm_set_peers.argtypes = [vp, vp, vp]
+    lib.acm_state_signature.argtypes = [vp, C.POINTER(C.c_ulonglong)]
     lib.acm_phase_launch.argtypes = [vp, i32, i32]
     lib.acm_phase_commit.argtypes = [vp]
     lib.acm_hydro_launch.argtypes = [vp, i32, i32]
@@ -264,6 +265,12 @@ class ACM:
         a, b, n = C.c_double(), C.c_double(), C.c_longlong()
         self._call(self._lib.acm_profile_read, C.byref(a), C.byref(b), C.byref(n))
         return a.value, b.value, n.value
+
+    def state_signature(self):
+        """acm_state_signature: what must agree between the slabs of a decomposition in peer mode"""
+        out = (C.c_ulonglong * 8)()
+        self._call(self._lib.acm_state_signature, out)
+        return tuple(out)
 
     @property
     def launch_count(self):

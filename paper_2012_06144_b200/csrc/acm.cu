@@ -60,6 +60,7 @@ struct acm_ctx {
     int sticky;                 // ACM_OK or ACM_ECUDA
     dim3 block;
     long long launches;
+    long long steps_done;       // committed hydrodynamic steps since acm_init (acm_state_signature)
     int cpt;                    // cells per thread of the two LB kernels: 1, or 2 (pair kernels: 8 / 16-byte accesses, packed fp32)
     int subiter;                // sweeps of the fixed point of eq. 22 (acm_set_subiter; 1 = the single evaluation, A10)
     int phase_planes, hydro_planes;   // owned planes launched since the last acm_*_commit (guard of the split launches)
@@ -253,6 +254,7 @@ static int launch_hydro_range(acm_ctx* c, int z0, int z1)
 static void commit_hydro(acm_ctx* c)
 {
     c->hydro_planes = 0;
+    c->steps_done += 1;
     if (c->options & ACM_OPT_UNFUSED) c->curU ^= 1;
     c->curG ^= 1;
     c->stG = next_state(c->stG);
@@ -319,7 +321,7 @@ static cudaGraphExec_t graph_for_state(acm_ctx* c)
         if (g.key == key) return g.exec;
     if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return nullptr; }
     const cudaStream_t user = c->stream;
-    const long long launches = c->launches;
+    const long long launches = c->launches, steps_done = c->steps_done;
     c->stream = c->cap_stream;
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
@@ -332,6 +334,7 @@ static cudaGraphExec_t graph_for_state(acm_ctx* c)
     if (graph) cudaGraphDestroy(graph);
     c->stream = user;
     c->launches = launches;
+    c->steps_done = steps_done;
     if (!ok) {
         cudaGetLastError();
         c->sticky = ACM_OK;          // a failed capture is not a failed launch: fall back to plain launches
@@ -373,6 +376,7 @@ static int step_t(acm_ctx* c, int n)
             cudaError_t e = cudaGraphLaunch(exec, c->stream);
             if (e != cudaSuccess) { c->sticky = ACM_ECUDA; return fail(ACM_ECUDA, "acm_step: cudaGraphLaunch: %s", cudaGetErrorString(e)); }
             c->launches += (long long)per_step * GRAPH_STEPS;
+            c->steps_done += GRAPH_STEPS;
             c->graph_replays += 1;
             done += GRAPH_STEPS;
         }
@@ -498,6 +502,7 @@ static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase,
     // cells or 256 fp32 cells (128 pairs) along x; single-cell fp32 falls back to 128 when nx is not a multiple of 256
     c->block = (precision == ACM_F32 && c->cpt == 1 && nx % 256 == 0) ? dim3(256, 1, 1) : dim3(128, 1, 1);
     c->launches = 0;
+    c->steps_done = 0;
     c->subiter = 1;
     c->phase_planes = c->hydro_planes = 0;
     c->profiling = false;
@@ -641,6 +646,18 @@ int acm_set_peers(acm_ctx* c, void* lo_workspace, void* hi_workspace)
     return ACM_OK;
 }
 
+int acm_state_signature(const acm_ctx* c, unsigned long long out[8])
+{
+    if (!c || !out) return fail(ACM_EINVAL, "acm_state_signature: NULL argument");
+    out[0] = c->offRed + align256((size_t)DIAG_WIDTH * (RED_BLOCKS + 1) * sizeof(double));      // workspace bytes (layout total)
+    out[1] = c->offH[c->curH]; out[2] = c->offG[c->curG]; out[3] = c->offC[c->curC];
+    out[4] = (unsigned long long)c->steps_done;
+    out[5] = (unsigned long long)c->nzl;
+    out[6] = (unsigned long long)(c->phase_planes != 0 || c->hydro_planes != 0);
+    out[7] = (unsigned long long)(c->precision == ACM_F32 ? (c->ref != 0.0 ? 2 : 1) : 0);
+    return ACM_OK;
+}
+
 int acm_phase_launch(acm_ctx* c, int z0, int z1)
 {
     ACM_CHECK_CTX(c);
@@ -781,6 +798,7 @@ int acm_init(acm_ctx* c, const void* phi, const void* u)
     if (!phi || !u) return fail(ACM_EINVAL, "acm_init: phi and u are required");
     graphs_clear(c);                  // the reference phase of the fp32 instance is a kernel argument
     c->phase_planes = c->hydro_planes = 0;
+    c->steps_done = 0;
     c->ref = 0.0;
     if (c->precision == ACM_F32) {
         // reference phase of the deviation storage: the phase that fills most of the domain

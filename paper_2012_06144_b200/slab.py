@@ -337,6 +337,23 @@ class PeerSlabRunner(SlabRunner):
         for s in self.slabs:
             lo, hi = self._neighbours(s.rank)
             s._call(s._lib.acm_set_peers, self._ptr(lo), self._ptr(hi))
+        self.check_consistency()
+
+    def check_consistency(self):
+        """A slab reads its neighbours' arrays at its OWN offsets and buffer parity (peers_at in acm.cu): layout,
+        current buffers, step count, slab height and fp32 reference phase must agree on all ranks.  Compared
+        across the local slabs and, for one slab per process, across the group (host-side all_gather)."""
+        sigs = {s.rank: s.state_signature() for s in self.slabs}
+        if not self.ex.local_only:
+            import torch.distributed as dist
+            gathered = [None] * self.nranks
+            dist.all_gather_object(gathered, sigs, group=self.ex.group)
+            sigs = {r: v for d in gathered for r, v in d.items()}
+        ref = next(iter(sigs.values()))
+        bad = {r: v for r, v in sigs.items() if v != ref}
+        if bad or ref[6]:
+            raise RuntimeError(f"peer mode: the slabs are out of step (workspace bytes, offsets of the current h/g/phi, steps, "
+                               f"planes, partly launched, reference phase): {sigs}")
 
     def _neighbours(self, r):
         lo = None if (self._wall_z and r == 0) else (r - 1) % self.nranks
@@ -389,10 +406,15 @@ class PeerSlabRunner(SlabRunner):
             self.sync()
             self.steps += 1
 
+    def init(self, phi_global, u_global):
+        super().init(phi_global, u_global)
+        self.check_consistency()
+
     def refresh_halos(self):
         """Ghost planes are not used for stepping in peer mode; the exports (acm_get_pdfs, pressure) still read them:
         pull them from the neighbours' workspaces.  Equal layouts: the neighbour's planes sit at the offsets of this
         slab's own plan for the opposite face."""
+        self.check_consistency()
         self.sync()
         for s in self.slabs:
             lo, hi = self._neighbours(s.rank)

@@ -125,8 +125,11 @@ def test_config2_scaled_walls_gravity_100_steps():
     gradients while theta is not small (compressibility moved phi 2e-4 off its bulk value), and the
     anti-diffusive forcing amplifies any 1-ulp difference by ~1e7 in 100 steps -- the oracle itself
     does that to a 1e-16 relative perturbation of its input.  The 100-step bound is therefore
-    1e-10 or 20x the oracle's own sensitivity to such a perturbation, whichever is larger; u, which
-    is not affected, keeps the plain 1e-10."""
+    1e-10 or 20x the oracle's own sensitivity to such a perturbation, whichever is larger -- but never
+    more than 1e-7, and the sensitivity itself must stay below 5e-9 (measured 1.3e-9), so that the bound
+    cannot grow without limit; u, which is not affected, keeps the plain 1e-10.  The same geometry with
+    a well-conditioned bulk is held to the plain 1e-10 by test_walls_well_conditioned_100_steps, and phi
+    itself is held to 1e-10 here wherever the oracle's own sensitivity stays below 1e-13."""
     p, phi, u = inputs.config2(nx=24, ny=48, nz=24, R=6.0, gy=-1e-6, centre=(12.0, 9.0, 12.0))
     o, a = _run_both(p, phi, u, 40, block=(32, 2, 2))
     _compare_fields(o, a, TOL_FIELD_100)
@@ -139,9 +142,14 @@ def test_config2_scaled_walls_gravity_100_steps():
     po, uo, _ = o.fields(False)
     p2, u2, _ = o2.fields(False)
     pa, ua, _ = a.fields(False)
-    own = np.abs(po - p2).max()
+    own_field = np.abs(po - p2)
+    own = own_field.max()
+    dphi = np.abs(pa.cpu().numpy() - po)
     assert np.abs(ua.cpu().numpy() - uo).max() <= TOL_FIELD_100
-    assert np.abs(pa.cpu().numpy() - po).max() <= max(TOL_FIELD_100, 20 * own), (own,)
+    assert own <= 5e-9, own
+    assert dphi.max() <= min(max(TOL_FIELD_100, 20 * own), 1e-7), (dphi.max(), own)
+    quiet = own_field <= 1e-13                 # cells the oracle itself reproduces: the plain bar
+    assert quiet.mean() > 0.5 and dphi[quiet].max() <= TOL_FIELD_100, (quiet.mean(), dphi[quiet].max())
     m0 = phi.sum()
     assert abs(a.phi_mass() - m0) / m0 < 1e-12
 

@@ -87,3 +87,74 @@ def test_config3_whole_grid_100_steps(config3_twin):
     mass = t.a.phi_mass()
     assert abs(mass - t.o.phi_mass()) <= 1e-12 * abs(mass)
     assert abs(mass - t.m0) <= 1e-12 * abs(t.m0)
+
+
+# ------------------------------------------------------------------------------------------
+# config 2 at full size: walls in y, gravity, one light bubble
+# ------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def config2_twin():
+    p, phi, u = inputs.config2()
+    t = _Twin(p, phi, u)
+    yield t
+    del t
+    torch.cuda.empty_cache()
+
+
+def test_config2_whole_grid_first_20_steps(config2_twin):
+    """Every element after 1 and 3 steps at the one-step bar; phi, u, p after 20 steps at the plain 1e-10 (observed
+    1e-14): up to there the run is well conditioned everywhere."""
+    t = config2_twin
+    for n in (1, 3):
+        t.advance_to(n)
+        dh, dg = t.pdf_diffs()
+        dphi, du, dp = t.field_diffs()
+        print(f"config 2, 128x512x128, step {n}: max|dh| {dh:.2e} |dg| {dg:.2e} |dphi| {dphi:.2e} |du| {du:.2e} |dp| {dp:.2e}")
+        for d in (dh, dg, dphi, du, dp):
+            assert d <= n * TOL_PDF_1STEP, (n, dh, dg, dphi, du, dp)
+    t.advance_to(20)
+    dphi, du, dp = t.field_diffs()
+    print(f"config 2, step 20: max|dphi| {dphi:.2e} |du| {du:.2e} |dp| {dp:.2e}")
+    assert dphi <= TOL_FIELD_100 and du <= TOL_FIELD_100 and dp <= TOL_FIELD_100, (dphi, du, dp)
+
+
+def test_config2_whole_grid_100_steps_conditioning_aware(config2_twin):
+    """After 100 steps the plain 1e-10 is NOT attainable on this configuration, for any implementation: where phi sits
+    a little off a bulk value (compressed liquid at the bottom wall, the tails of the tanh profile around the bubble)
+    and its gradient is at rounding level, the unit normal of eq. 5 turns rounding noise into an O(theta) flux
+    (DESIGN.md "Conditioning").  The oracle shows it against itself: a second oracle run whose input differs by
+    1e-16 relative (`own`) drifts from the first by 1e-5 in phi in those regions.  So the bound is made per y-plane
+    from the oracle's own sensitivity: max(1e-10, 100 x own) with `own` taken over the plane and its 8 neighbours
+    on either side; planes the twin leaves below 1e-12 are held to the plain 1e-10, and they must be the majority.
+    Global caps keep the test from passing on garbage: 1e-4 on phi (the saturation level ~ theta), 1e-8 on u and p."""
+    t = config2_twin
+    p = t.p
+    rng = np.random.Generator(np.random.PCG64(1))
+    _, phi, u = inputs.config2()
+    twin = Oracle.from_params(p)
+    twin.init(phi * (1.0 + 1e-16 * rng.uniform(-1.0, 1.0, size=phi.shape)), u)
+    twin.step(100)
+    t.advance_to(100)
+    fo = t.o.fields()
+    ft = twin.fields()
+    fa = t.a.fields()
+    del twin
+    names = ("phi", "u", "p")
+    caps = (1e-4, 1e-8, 1e-8)
+    well = np.ones(p.ny, dtype=bool)
+    for name, cap, o_, t_, a_ in zip(names, caps, fo, ft, fa):
+        ax = (0, 2) if o_.ndim == 3 else (0, 1, 3)
+        own = np.abs(o_ - t_).max(axis=ax)
+        got = np.abs(a_.cpu().numpy() - o_).max(axis=ax)
+        own_w = np.array([own[max(0, y - 8): y + 9].max() for y in range(p.ny)])
+        bound = np.maximum(TOL_FIELD_100, 100.0 * own_w)
+        worst = int(np.argmax(got / bound))
+        print(f"config 2, step 100, {name}: max|d| {got.max():.2e} (oracle vs its 1e-16 twin: {own.max():.2e}); "
+              f"planes with own <= 1e-12: {(own_w <= 1e-12).sum()} of {p.ny}; worst plane y={worst}: {got[worst]:.2e} vs bound {bound[worst]:.2e}")
+        assert (got <= bound).all(), (name, worst, got[worst], bound[worst])
+        assert got.max() <= cap, (name, got.max())
+        well &= own_w <= 1e-12
+    assert well.sum() >= 0.6 * p.ny            # most of the domain is well conditioned, and there the plain bar holds
+    mass = t.a.phi_mass()
+    assert abs(mass - t.o.phi_mass()) <= 1e-12 * abs(mass)
+    assert abs(mass - t.m0) <= 1e-12 * abs(t.m0)
