@@ -77,6 +77,7 @@ class ClockSampler:
 
     def __init__(self, index):
         self.samples, self.reasons, self.max_mhz, self._stop = [], set(), None, threading.Event()
+        self.power, self.mem = [], []
         self._thread = None
         try:
             import pynvml
@@ -92,6 +93,11 @@ class ClockSampler:
         while not self._stop.is_set():
             try:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                    self.mem.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_MEM))
+                except Exception:
+                    pass
                 try:
                     r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
                 except Exception:
@@ -115,8 +121,11 @@ class ClockSampler:
             self._thread.join()
 
     def summary(self):
-        s = sorted(self.samples)
+        s, pw, mm = sorted(self.samples), sorted(self.power), sorted(self.mem)
         return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
+                "sm_mhz_first_last": [self.samples[0], self.samples[-1]] if s else None,
+                "mem_mhz": mm[len(mm) // 2] if mm else None,
+                "power_w": pw[len(pw) // 2] if pw else None, "power_w_max": pw[-1] if pw else None,
                 "reasons": sorted(self.reasons), "samples": len(s)}
 
 
@@ -245,9 +254,11 @@ def measure(args, config, precision, dev, local_rank, world, K, W, with_e2e=True
     u_h = torch.from_numpy(u.astype(np_dtype)).pin_memory()
     sim = ACM.from_params(p, precision=precision, device=dev, inplace=args.inplace, unfused=args.unfused)
     if args.cpt:
-        sim.set_cells_per_thread(args.cpt)
+        sim.set_cells_per_thread(*args.cpt)
     if args.block:
         sim.set_block(*args.block)
+    if args.graph is not None:
+        sim.set_graph(args.graph)
     sim.init(phi_h.to(dev), u_h.to(dev))
     N = p.ncells
     b_phase, b_hydro = bytes_per_cell(p.stencil_phase, p.stencil_hydro, esz)
@@ -263,6 +274,7 @@ def measure(args, config, precision, dev, local_rank, world, K, W, with_e2e=True
             ev[r + 1].record()
         replicas.barrier(dev)
     launches = (sim.launch_count - launches0) // REPEATS
+    graph_replays = sim.graph_replays
     intervals = sorted(replicas.max_over_ranks(ev[r].elapsed_time(ev[r + 1]), dev) for r in range(REPEATS))
     ms = intervals[REPEATS // 2]
     value = replicas.aggregate_mlups(N, K, ms, world)
@@ -277,7 +289,7 @@ def measure(args, config, precision, dev, local_rank, world, K, W, with_e2e=True
 
     res = {"p": p, "phi": phi, "u": u, "name": name, "N": N, "esz": esz, "value": value, "ms": ms, "intervals": intervals,
            "value_min": replicas.aggregate_mlups(N, K, intervals[-1], world), "value_max": replicas.aggregate_mlups(N, K, intervals[0], world),
-           "phase_ms": phase_ms, "hydro_ms": hydro_ms, "launches": launches, "mass": mass, "clocks": clk.summary(),
+           "phase_ms": phase_ms, "hydro_ms": hydro_ms, "launches": launches, "graph_replays": graph_replays, "mass": mass, "clocks": clk.summary(),
            "b_phase": b_phase, "b_hydro": b_hydro}
 
     if with_e2e:
@@ -358,7 +370,7 @@ def run_acm(args, rank, local_rank, world):
                              "of state streamed every step vs 126 MB L2",
                        "bytes_per_cell": {"phase": r["b_phase"], "hydro": r["b_hydro"]},
                        "step_algorithmic_GBps": step_gbs, "step_frac_of_peak": step_gbs / peak, "step_frac_of_nominal": step_gbs / NOMINAL_HBM_GBS,
-                       "phase_ms": r["phase_ms"], "hydro_ms": r["hydro_ms"],
+                       "phase_ms": r["phase_ms"], "hydro_ms": r["hydro_ms"], "cuda_graph_replays": r["graph_replays"],
                        "sum_phi": r["mass"], "finite": r["finite"]},
             "clocks": r["clocks"],
             "e2e": {"value": r["e2e"], "unit": UNIT, "h2d_bytes_per_step": 4 * N * esz / K,
@@ -489,7 +501,9 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--block", type=int, nargs=3, default=None)
-    ap.add_argument("--cpt", type=int, default=0, choices=[0, 1, 2], help="cells per thread of the LB kernels (0 = the library's default)")
+    ap.add_argument("--cpt", type=int, nargs=2, default=None, metavar=("PHASE", "HYDRO"),
+                    help="cells per thread of the phase / hydro kernel: 1, 2, or 0 = the library's default")
+    ap.add_argument("--graph", type=int, default=None, choices=[-1, 0, 1], help="CUDA graphs in acm_step: -1 automatic (small grids), 0 never, 1 always")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the extra fp32 config-5 measurement of the default run")
     ap.add_argument("--inplace", action="store_true", help="in-place AA streaming (one grid per population set)")

@@ -283,12 +283,13 @@ int acm_run_host(acm_ctx*, const void* phi_host, const void* u_host, int n,
  * Optional; the defaults are tuned for B200.  ACM_ESTATE while a step is partly launched. */
 int acm_set_block(acm_ctx*, int bx, int by, int bz);
 
-/* Cells per thread of the two LB kernels: 1, or 2 = the pair kernels, in which a thread updates two x-adjacent
- * cells with 8-byte (fp32) / 16-byte (fp64) accesses wherever the pair stays aligned (own cell, directions with
- * e_x = 0) and, for fp32, Blackwell's packed fp32 arithmetic (FADD2 / FMUL2 / FFMA2: one instruction per pair).
- * Default: 2 for ACM_F32 when nx is even, 1 for ACM_F64.  Same results up to rounding order.  A block of
- * acm_set_block then covers 2 bx cells of a row.  ACM_EINVAL for n = 2 with odd nx or ACM_OPT_UNFUSED. */
-int acm_set_cells_per_thread(acm_ctx*, int n);
+/* Cells per thread of the phase-field / the hydrodynamic LB kernel: 1, or 2 = the pair kernels, in which a thread
+ * updates two x-adjacent cells with 8-byte (fp32) / 16-byte (fp64) accesses wherever the pair stays aligned (own cell,
+ * directions with e_x = 0) and, for fp32, Blackwell's packed fp32 arithmetic (FADD2 / FMUL2 / FFMA2: one instruction
+ * per pair); 0 = the library's default for that kernel: 2 when nx is even and the kernel is fp32, or fp64 with a
+ * lattice of at most 19 directions (hydrodynamic kernel: D3Q15 / D3Q19 only), else 1 (measured).  Same results up to rounding order.  A block of acm_set_block then
+ * covers 2 bx cells of a row.  ACM_EINVAL for 2 with odd nx or ACM_OPT_UNFUSED. */
+int acm_set_cells_per_thread(acm_ctx*, int phase, int hydro);
 
 /* Per-kernel device timing for the roofline report.  acm_profile(ctx, 1) makes every later
  * acm_step record CUDA events on the stream around each of its two kernels (and drops earlier

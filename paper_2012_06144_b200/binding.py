@@ -5,6 +5,7 @@ library's CUDA kernels.  There is no fallback: a missing library or a missing GP
 """
 from __future__ import annotations
 
+import contextlib
 import ctypes as C
 import os
 
@@ -82,7 +83,7 @@ def load(build_if_missing: bool = True):
     lib.acm_drag_exp.restype = dbl
     lib.acm_set_block.argtypes = [vp, i32, i32, i32]
     lib.acm_set_subiter.argtypes = [vp, i32]
-    lib.acm_set_cells_per_thread.argtypes = [vp, i32]
+    lib.acm_set_cells_per_thread.argtypes = [vp, i32, i32]
     lib.acm_set_graph.argtypes = [vp, i32]
     lib.acm_graph_replays.argtypes = [vp]
     lib.acm_graph_replays.restype = C.c_longlong
@@ -182,6 +183,28 @@ class ACM:
         with torch.cuda.device(self.device):
             _check(self._lib, fn(self._h, *args))
 
+    @contextlib.contextmanager
+    def _on_stream(self, *inputs):
+        """libacm enqueues on self.stream; torch allocates and the caller computes on torch's CURRENT stream.  When the
+        two differ: self.stream first waits for the current stream (inputs are complete before the library reads
+        them; their memory is not recycled while it does: record_stream), outputs are allocated under self.stream,
+        and the current stream waits for self.stream afterwards (outputs are complete before the caller reads them)."""
+        cur = torch.cuda.current_stream(self.device)
+        same = cur.cuda_stream == self.stream.cuda_stream
+        if not same:
+            self.stream.wait_stream(cur)
+            for t in inputs:
+                if t is not None:
+                    t.record_stream(self.stream)
+        outputs = []
+        with torch.cuda.stream(self.stream):
+            yield outputs
+        if not same:
+            cur.wait_stream(self.stream)
+            for t in outputs:          # allocated under self.stream, read by the caller on `cur`
+                if t is not None:
+                    t.record_stream(cur)
+
     def _dev(self, t, shape):
         assert t.is_cuda and t.dtype == self.dtype and t.is_contiguous() and tuple(t.shape) == tuple(shape), \
             (t.device, t.dtype, t.shape, shape)
@@ -196,9 +219,10 @@ class ACM:
     def set_block(self, bx, by=1, bz=1):
         self._call(self._lib.acm_set_block, int(bx), int(by), int(bz))
 
-    def set_cells_per_thread(self, n):
-        """1, or 2 = pair kernels (8/16-byte accesses, packed fp32 arithmetic); default 2 for f32 with even nx"""
-        self._call(self._lib.acm_set_cells_per_thread, int(n))
+    def set_cells_per_thread(self, phase, hydro=None):
+        """cells per thread of the phase / hydro kernel: 1, 2 = pair kernels (8/16-byte accesses, packed fp32
+        arithmetic), 0 = the library's default (2 for fp32 and for fp64 lattices up to D3Q19, when nx is even)"""
+        self._call(self._lib.acm_set_cells_per_thread, int(phase), int(phase if hydro is None else hydro))
 
     def set_subiter(self, sweeps):
         """sweeps of the fixed point of eq. 22 (1 = single evaluation of F_mu with the previous velocity)"""
@@ -217,16 +241,19 @@ class ACM:
         self._call(self._lib.acm_set_reference_phase, int(phase))
 
     def init(self, phi, u):
-        self._call(self._lib.acm_init, self._dev(phi, self.shape), self._dev(u, (3,) + self.shape))
+        with self._on_stream(phi, u):
+            self._call(self._lib.acm_init, self._dev(phi, self.shape), self._dev(u, (3,) + self.shape))
 
     def step(self, n=1):
         self._call(self._lib.acm_step, int(n))
 
     def fields(self, want_p=True):
-        phi = torch.empty(self.shape, dtype=self.dtype, device=self.device)
-        u = torch.empty((3,) + self.shape, dtype=self.dtype, device=self.device)
-        p = torch.empty(self.shape, dtype=self.dtype, device=self.device) if want_p else None
-        self._call(self._lib.acm_fields, _ptr(phi), _ptr(u), _ptr(p))
+        with self._on_stream() as outs:
+            phi = torch.empty(self.shape, dtype=self.dtype, device=self.device)
+            u = torch.empty((3,) + self.shape, dtype=self.dtype, device=self.device)
+            p = torch.empty(self.shape, dtype=self.dtype, device=self.device) if want_p else None
+            self._call(self._lib.acm_fields, _ptr(phi), _ptr(u), _ptr(p))
+            outs += [phi, u, p]
         return phi, u, p
 
     def phi_mass(self):
@@ -241,15 +268,18 @@ class ACM:
         return out[0], tuple(out[1:4]), tuple(out[4:7])
 
     def get_pdfs(self):
-        h = torch.empty((self.Qh,) + self.shape, dtype=self.dtype, device=self.device)
-        g = torch.empty((self.Qg,) + self.shape, dtype=self.dtype, device=self.device)
-        self._call(self._lib.acm_get_pdfs, _ptr(h), _ptr(g))
+        with self._on_stream() as outs:
+            h = torch.empty((self.Qh,) + self.shape, dtype=self.dtype, device=self.device)
+            g = torch.empty((self.Qg,) + self.shape, dtype=self.dtype, device=self.device)
+            self._call(self._lib.acm_get_pdfs, _ptr(h), _ptr(g))
+            outs += [h, g]
         return h, g
 
     def set_pdfs(self, h=None, g=None):
         hp = None if h is None else self._dev(h, (self.Qh,) + self.shape)
         gp = None if g is None else self._dev(g, (self.Qg,) + self.shape)
-        self._call(self._lib.acm_set_pdfs, hp, gp)
+        with self._on_stream(h, g):
+            self._call(self._lib.acm_set_pdfs, hp, gp)
 
     def run_host(self, phi_host, u_host, n, phi_out=None, u_out=None, p_out=None):
         """Host buffers in (CPU tensors, ideally pinned), host buffers out; transfers inside."""

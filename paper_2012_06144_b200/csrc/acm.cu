@@ -61,7 +61,7 @@ struct acm_ctx {
     dim3 block;
     long long launches;
     long long steps_done;       // committed hydrodynamic steps since acm_init (acm_state_signature)
-    int cpt;                    // cells per thread of the two LB kernels: 1, or 2 (pair kernels: 8 / 16-byte accesses, packed fp32)
+    int cpt_phase, cpt_hydro;   // cells per thread of the two LB kernels: 1, or 2 (pair kernels: 8 / 16-byte accesses, packed fp32)
     int subiter;                // sweeps of the fixed point of eq. 22 (acm_set_subiter; 1 = the single evaluation, A10)
     int phase_planes, hydro_planes;   // owned planes launched since the last acm_*_commit (guard of the split launches)
     // optional per-kernel timing (acm_profile): events recorded around every LB kernel.  The events come from a pool
@@ -128,7 +128,7 @@ static int check_launch(acm_ctx* c, const char* what, cudaError_t e, int count =
 // Launch geometry of the two LB kernels: x-rows tiled by the block, or -- when the block is 1-D and
 // nx is not a multiple of it (e.g. the paper's 260^3) -- a linear launch over all cells.
 // (with two cells per thread a row has nx / 2 pairs)
-static bool lb_linear(const acm_ctx* c) { return c->block.y == 1 && c->block.z == 1 && (c->nx / c->cpt) % (int)c->block.x != 0; }
+static bool lb_linear(const acm_ctx* c, int cpt) { return c->block.y == 1 && c->block.z == 1 && (c->nx / cpt) % (int)c->block.x != 0; }
 
 // geometry block of a launch over the owned planes [z0, z1) (relative to the first owned plane)
 static Geom geom_of(const acm_ctx* c, bool linear, int z0, int z1)
@@ -154,7 +154,7 @@ static Launch launch_over(const acm_ctx* c, dim3 b, bool linear, int nplanes, in
     return Launch{dim3((nxe + b.x - 1) / b.x, (c->ny + b.y - 1) / b.y, (nplanes + b.z - 1) / b.z), b, c->stream};
 }
 
-static Launch lb_launch(const acm_ctx* c, int nplanes) { return launch_over(c, c->block, lb_linear(c), nplanes, c->cpt); }
+static Launch lb_launch(const acm_ctx* c, int nplanes, int cpt) { return launch_over(c, c->block, lb_linear(c, cpt), nplanes, cpt); }
 
 template <typename T> static T* wsp(acm_ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }
 
@@ -197,7 +197,8 @@ static int launch_phase_range(acm_ctx* c, int z0, int z1)
     a.Hsrc = wsp<T>(c, c->offH[c->curH]); a.Hdst = wsp<T>(c, c->offH[c->curH ^ 1]);
     a.Csrc = wsp<T>(c, c->offC[c->curC]); a.Cdst = wsp<T>(c, c->offC[c->curC ^ 1]);
     a.U = wsp<T>(c, c->offU[c->curU]);
-    a.g = geom_of(c, lb_linear(c), z0, z1);
+    const int cpt = (c->options & ACM_OPT_UNFUSED) ? 1 : c->cpt_phase;
+    a.g = geom_of(c, lb_linear(c, cpt), z0, z1);
     a.N = (unsigned)c->N;
     const double omega = 1.0 / (3.0 * c->M + 0.5);     // tau_phi = M/c_s^2 (eq. 2), shifted by 1/2
     a.one_minus_omega = (T)(1.0 - omega);
@@ -205,11 +206,11 @@ static int launch_phase_range(acm_ctx* c, int z0, int z1)
     a.ref = (T)c->ref;
     a.Hpeer = peers_at<T>(c, c->offH[c->curH]);
     a.Cpeer = peers_at<T>(c, c->offC[c->curC]);
-    const Launch l = lb_launch(c, z1 - z0);
+    const Launch l = lb_launch(c, z1 - z0, cpt);
     const int coll = (c->options & ACM_OPT_PHASE_SRT) ? PHASE_SRT : PHASE_MRT;
     const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
     cudaError_t e = unfused ? launch_unfused_phase<T>(c->Qh, c->walls != 0, coll, l, a)
-                    : c->cpt == 2 ? launch_phase2<T>(c->Qh, c->walls != 0, c->stH, coll, l, a)
+                    : cpt == 2 ? launch_phase2<T>(c->Qh, c->walls != 0, c->stH, coll, l, a)
                                   : launch_phase<T>(c->Qh, c->walls != 0, c->stH, coll, l, a);
     c->phase_planes += z1 - z0;
     return check_launch(c, unfused ? "stream_h/phi/collide_h kernels" : "phase_kernel", e, unfused ? 3 : 1);
@@ -230,7 +231,8 @@ static int launch_hydro_range(acm_ctx* c, int z0, int z1)
     a.Gsrc = wsp<T>(c, c->offG[c->curG]); a.Gdst = wsp<T>(c, c->offG[c->curG ^ 1]);
     a.C = wsp<T>(c, c->offC[c->curC]);
     a.U = wsp<T>(c, c->offU[c->curU]);
-    a.g = geom_of(c, lb_linear(c), z0, z1);
+    const int cpt = (c->options & ACM_OPT_UNFUSED) ? 1 : c->cpt_hydro;
+    a.g = geom_of(c, lb_linear(c, cpt), z0, z1);
     a.N = (unsigned)c->N;
     // rho and tau at the reference phase of the stored phi (ref = 0: the light phase, as in eqs. 8, 20)
     a.ref = (T)c->ref;
@@ -242,10 +244,10 @@ static int launch_hydro_range(acm_ctx* c, int z0, int z1)
     a.subiter = c->subiter;
     a.Gpeer = peers_at<T>(c, c->offG[c->curG]);
     a.Cpeer = peers_at<T>(c, c->offC[c->curC]);
-    const Launch l = lb_launch(c, z1 - z0);
+    const Launch l = lb_launch(c, z1 - z0, cpt);
     const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
     cudaError_t e = unfused ? launch_unfused_hydro<T>(c->Qg, c->walls != 0, l, a, wsp<T>(c, c->offU[c->curU]), wsp<T>(c, c->offU[c->curU ^ 1]))
-                    : c->cpt == 2 ? launch_hydro2<T>(c->Qg, c->walls != 0, c->stG, l, a)
+                    : cpt == 2 ? launch_hydro2<T>(c->Qg, c->walls != 0, c->stG, l, a)
                                   : launch_hydro<T>(c->Qg, c->walls != 0, c->stG, l, a);
     c->hydro_planes += z1 - z0;
     return check_launch(c, unfused ? "stream_g/velocity/collide_g kernels" : "hydro_kernel", e, unfused ? 3 : 1);
@@ -439,6 +441,22 @@ static int copy_field_shifted(acm_ctx* c, void* dst, const void* src, size_t n, 
     if (!(c)) return fail(ACM_EINVAL, "%s: NULL context", __func__);              \
     if ((c)->sticky) return fail(ACM_ECUDA, "%s: context has a sticky CUDA error", __func__)
 
+// Default cells per thread and block.  fp32: two cells per thread (8-byte accesses, packed fp32 arithmetic) whenever
+// the rows allow it.  fp64: the pairing (16-byte accesses) saves index arithmetic, hence power: +1.8 % at D3Q15 / D3Q19
+// under the sustained 1 kW power cap, nothing in a burst, while the 250 registers of a D3Q27 pair cost 2-5 % and the
+// D2Q9 hydrodynamic pair 6 % (profiles/r2_profiles.md) -- so two cells for the phase kernel up to D3Q19 and for the
+// hydrodynamic kernel at D3Q15 / D3Q19, one otherwise.
+// One block = 1 KB of every population row (measured best on B200 for both precisions, profiles/): 128 fp64 cells or
+// 256 fp32 cells (128 pairs) along x; single-cell fp32 falls back to 128 when nx is not a multiple of 256.
+static void default_cells_per_thread(acm_ctx* c)
+{
+    const bool can_pair = c->nx % 2 == 0 && !(c->options & ACM_OPT_UNFUSED);
+    const bool f32 = c->precision == ACM_F32;
+    c->cpt_phase = (can_pair && (f32 || c->Qh <= 19)) ? 2 : 1;
+    c->cpt_hydro = (can_pair && (f32 || c->Qg == 15 || c->Qg == 19)) ? 2 : 1;
+    c->block = (f32 && c->cpt_phase == 1 && c->nx % 256 == 0) ? dim3(256, 1, 1) : dim3(128, 1, 1);
+}
+
 // nz = owned planes; rank/nranks/nz_global/zglob0 describe the slab (nranks = 0: a plain context without ghost planes)
 static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int stencil_hydro, double rho_H, double rho_L,
                        double sigma, double xi, double M, double nu_H, double nu_L, const double gravity[3], unsigned wall_flags,
@@ -495,12 +513,7 @@ static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase,
     c->stH = c->stG = ST_POST;
     c->initialised = false;
     c->sticky = ACM_OK;
-    // fp32: two cells per thread (8-byte accesses, packed fp32 arithmetic) whenever the rows allow it; fp64: one
-    // (the 16-byte pairing is a measured wash; acm_set_cells_per_thread switches either)
-    c->cpt = (precision == ACM_F32 && nx % 2 == 0 && !(options & ACM_OPT_UNFUSED)) ? 2 : 1;
-    // one block = 1 KB of every population row (measured best on B200 for both precisions, profiles/): 128 fp64
-    // cells or 256 fp32 cells (128 pairs) along x; single-cell fp32 falls back to 128 when nx is not a multiple of 256
-    c->block = (precision == ACM_F32 && c->cpt == 1 && nx % 256 == 0) ? dim3(256, 1, 1) : dim3(128, 1, 1);
+    default_cells_per_thread(c);
     c->launches = 0;
     c->steps_done = 0;
     c->subiter = 1;
@@ -756,14 +769,18 @@ int acm_set_block(acm_ctx* c, int bx, int by, int bz)
     return ACM_OK;
 }
 
-int acm_set_cells_per_thread(acm_ctx* c, int n)
+int acm_set_cells_per_thread(acm_ctx* c, int phase, int hydro)
 {
     ACM_CHECK_CTX(c);
-    if (n != 1 && n != 2) return fail(ACM_EINVAL, "acm_set_cells_per_thread: 1 or 2");
-    if (n == 2 && (c->nx % 2 != 0 || (c->options & ACM_OPT_UNFUSED)))
+    if (phase < 0 || phase > 2 || hydro < 0 || hydro > 2) return fail(ACM_EINVAL, "acm_set_cells_per_thread: 0 (default), 1 or 2");
+    if ((phase == 2 || hydro == 2) && (c->nx % 2 != 0 || (c->options & ACM_OPT_UNFUSED)))
         return fail(ACM_EINVAL, "acm_set_cells_per_thread: two cells per thread need an even nx and the fused kernels");
     if (c->phase_planes || c->hydro_planes) return fail(ACM_ESTATE, "acm_set_cells_per_thread: a step is partly launched (commit it first)");
-    c->cpt = n;
+    const dim3 block = c->block;
+    default_cells_per_thread(c);
+    c->block = block;
+    if (phase) c->cpt_phase = phase;
+    if (hydro) c->cpt_hydro = hydro;
     graphs_clear(c);
     return ACM_OK;
 }

@@ -205,3 +205,28 @@ def test_commit_guards():
     b.step(1)
     for x, y in zip(a.get_pdfs() + a.fields(), b.get_pdfs() + b.fields()):
         assert torch.equal(x, y)
+
+
+def test_context_on_a_side_stream_while_the_caller_uses_another():
+    """libacm enqueues on the stream given to acm_create; the caller's tensors live on torch's current stream.  The
+    binding orders the two (inputs complete before the library reads them, outputs complete before the caller does)."""
+    from paper_2012_06144_b200.binding import ACM
+    p, phi, u = inputs.scaled_config3(32)
+    side = torch.cuda.Stream()
+    a = ACM.from_params(p, stream=side)                 # current stream stays the default one
+    big = torch.randn(4096, 4096, device="cuda")
+    for _ in range(3):
+        big = big @ big * 1e-4                          # keep the current stream busy while the inputs are produced on it
+    phi_d = _dev(phi) + 0.0 * big[0, 0].double()
+    u_d = _dev(u) + 0.0 * big[1, 1].double()
+    a.init(phi_d, u_d)
+    del phi_d, u_d
+    a.step(10)
+    c, uu, pr = a.fields()
+    h, g = a.get_pdfs()
+    got = [t.clone() for t in (c, uu, pr, h, g)]        # reads on the current stream
+    b = _acm(p)
+    b.init(_dev(phi), _dev(u))
+    b.step(10)
+    for x, y in zip(got, b.fields() + b.get_pdfs()):
+        assert torch.equal(x, y)
