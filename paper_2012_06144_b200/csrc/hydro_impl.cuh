@@ -15,7 +15,7 @@ namespace acm {
 // ------------------------------------------------------------------------------------------
 // HVAR = 1: the operator variants of lb_math.cuh (bulk moment relaxed with 1, sub-iterated velocity), switched by a.bulk_one / a.subiter
 template <typename T, int Q, bool WALLS, int STATE, bool PEER = false, int HVAR = 0>
-__global__ void __launch_bounds__(ACM_MAXT, ACM_HYDRO_MINB) hydro_kernel(const HydroArgs<T> a)
+__global__ void __launch_bounds__(ACM_MAXT, (WALLS && ACM_HYDRO_MINB > 2) ? 2 : ACM_HYDRO_MINB) hydro_kernel(const HydroArgs<T> a)
 {
     int x, y, z;
     if (!cell_of_thread(a.g, x, y, z)) return;

@@ -12,7 +12,7 @@ namespace acm {
 // With d = j - phi_new u + (theta/6) n:   h*_i = h^eq_i + F_i/2 + (1-omega_phi) 3 w_i e_i.d
 // ------------------------------------------------------------------------------------------
 template <typename T, int Q, bool WALLS, int STATE, int COLL, bool PEER = false>
-__global__ void __launch_bounds__(ACM_MAXT, ACM_PHASE_MINB) phase_kernel(const PhaseArgs<T> a)
+__global__ void __launch_bounds__(ACM_MAXT, (WALLS && ACM_PHASE_MINB > 2) ? 2 : ACM_PHASE_MINB) phase_kernel(const PhaseArgs<T> a)
 {
     int x, y, z;
     if (!cell_of_thread(a.g, x, y, z)) return;
