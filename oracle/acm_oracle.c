@@ -49,7 +49,8 @@
  * orthogonality of M, eq.25 forcing identity, brute-force 4^3 step against a
  * hand-expanded projector form, FD operators on polynomials, sum(phi)
  * conservation, uniform state, Galilean invariance, planar tanh profile
- * (eq. 3), mobility and viscosity decay rates, Poiseuille profile, Laplace law;
+ * (eq. 3) and its advection with a uniform flow (eq. 1), mobility and viscosity decay rates, Poiseuille profile,
+ * Laplace law;
  * variants (tests/test_oracle_variants.py, test_oracle_d2q9.py): SRT brute force and omega = 1
  * special case, bubble diagnostics (symmetry, translation, continuum volume), eqs. 31-35
  * round trip, D2Q9 lattice identities / brute force / transport limits; A26: brute force with the

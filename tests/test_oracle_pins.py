@@ -269,6 +269,38 @@ def test_planar_interface_stationary():
     assert np.abs(uu).max() < 1e-5
 
 
+@pytest.mark.parametrize("rho_L,sigma,u0", [(1.0, 0.0, 0.02), (1.0, 0.0, -0.05), (1e-3, 1e-4, 0.02)])
+def test_interface_is_advected_with_the_flow(rho_L, sigma, u0):
+    """eq. 1: d phi/dt + div(phi u) = (a term that vanishes on the equilibrium profile), so in a uniform flow
+    the slab of eq. 3 translates with u: after T steps both phi = 1/2 crossings have moved by u0 T (across the
+    periodic seam), within 0.5 % (measured lag 0.2 %), the flow stays uniform and sum(phi) is conserved.  A dropped or
+    mis-signed u in h^eq (eq. 6) changes the displacement by O(1)."""
+    p = Params(nx=64, ny=2, nz=2, rho_L=rho_L, sigma=sigma)
+    x = np.arange(64) + 0.5
+    prof = 0.5 * (np.tanh(2 * (x - 16) / p.xi) - np.tanh(2 * (x - 48) / p.xi))
+    phi = np.broadcast_to(prof[None, None, :], p.shape).copy()
+    u = inputs.zeros_u(p)
+    u[0] = u0
+    o = Oracle.from_params(p)
+    o.init(phi, u)
+    T = 500
+    o.step(T)
+    ph, uu, _ = o.fields(want_p=False)
+    line = ph[0, 0]
+
+    def crossing(lo):
+        idx = [(lo + k) % 64 for k in range(32)]
+        seg = line[idx]
+        k = int(np.argmax((seg[:-1] - 0.5) * (seg[1:] - 0.5) <= 0))
+        return x[idx[k]] + (0.5 - seg[k]) / (seg[k + 1] - seg[k])
+
+    for x0 in (16.0, 48.0):
+        moved = (crossing(int(x0 + u0 * T) - 15) - x0 + 32.0) % 64.0 - 32.0
+        assert abs(moved / (u0 * T) - 1.0) < 5e-3, (x0, moved)
+    assert np.abs(uu[0] - u0).max() < 2e-5 and np.abs(uu[1:]).max() < 1e-12
+    assert abs(ph.sum() / phi.sum() - 1.0) < 1e-12
+
+
 @pytest.mark.parametrize("Mob", [0.02, 0.08])
 def test_mobility_sine_decay(Mob):
     """eq. 2 + A2: with the interface term switched off (xi -> inf) and u = 0 the phase
