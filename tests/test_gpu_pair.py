@@ -132,3 +132,31 @@ def test_default_rule_and_argument_checks():
     assert a._lib.acm_set_cells_per_thread(a._h, 3, 1) == binding.ACM_EINVAL
     b = ACM.from_params(Params(nx=32, ny=4, nz=4), unfused=True)
     assert b._lib.acm_set_cells_per_thread(b._h, 2, 2) == binding.ACM_EINVAL          # Algorithm 1 has single-cell kernels only
+
+
+def test_pair_against_single_cell_on_seeded_random_shapes():
+    """Differential check on 16 seeded random grids / lattices / walls / options / blocks: the pair kernels against the
+    single-cell kernels over 3 steps (both are tied to the oracle above; this sweeps shapes no table lists)."""
+    rng = np.random.Generator(np.random.PCG64(2012))
+    for case in range(16):
+        nx = 2 * int(rng.integers(1, 90))
+        ny, nz = int(rng.integers(1, 9)), int(rng.integers(1, 9))
+        Qh, Qg = int(rng.choice([15, 19, 27])), int(rng.choice([15, 19, 27]))
+        walls = int(rng.integers(0, 8))
+        opts = dict(inplace=bool(rng.integers(0, 2)), phase_srt=bool(rng.integers(0, 2)), bulk_one=bool(rng.integers(0, 2)),
+                    subiter=int(rng.integers(1, 4)))
+        bx = int(rng.choice([8, 32, 64, 128]))
+        by = int(rng.choice([1, 2]))
+        p = Params(nx=nx, ny=ny, nz=nz, stencil_phase=Qh, stencil_hydro=Qg, wall_flags=walls, gravity=(1e-5, -2e-5, 1e-5),
+                   rho_L=0.05, sigma=2e-3, nu_H=0.05, nu_L=0.2)
+        phi, u, h, g = random_state(p, seed=100 + case)
+        out = []
+        for cpt in ((1, 1), (2, 2)):
+            a = _acm(p, cpt, **opts)
+            a.set_block(bx, by, 1)
+            a.init(_dev(phi), _dev(u))
+            a.set_pdfs(_dev(h), _dev(g))
+            a.step(3)
+            out.append(a.get_pdfs() + a.fields())
+        for x, y in zip(*out):
+            assert float((x - y).abs().max()) <= 3 * TOL_PDF_1STEP, (case, nx, ny, nz, Qh, Qg, walls, opts, bx, by)
