@@ -222,6 +222,22 @@ def workload_name_only(config):
     return None, None, None, names[config]
 
 
+def dist_backend():
+    """"nccl" (one rank per GPU).  ACM_DIST_BACKEND=gloo lets the multi-rank flow be exercised on a box with fewer
+    GPUs than ranks (tests/test_gpu_bench_flow.py): the ranks then share GPUs and only host tensors are reduced."""
+    return os.environ.get("ACM_DIST_BACKEND", "nccl")
+
+
+def pick_device(local_rank):
+    import torch
+    n = torch.cuda.device_count()
+    if dist_backend() == "nccl" and local_rank >= n:
+        raise SystemExit(f"bench.py: local rank {local_rank} has no GPU ({n} visible)")
+    local_rank = local_rank % n
+    torch.cuda.set_device(local_rank)
+    return local_rank, torch.device("cuda", local_rank)
+
+
 NOMINAL_HBM_GBS = 8000.0      # vendor figure for context (B200_PROFILING.md: 7.7 TB/s HGX, 8 TB/s DGX)
 REPEATS = 5
 
@@ -334,9 +350,8 @@ def run_acm(args, rank, local_rank, world):
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    replicas.init("nccl", dev)
+    local_rank, dev = pick_device(local_rank)
+    replicas.init(dist_backend(), dev)
 
     K, W = args.steps, max(args.warmup, 20)      # never fewer than 20 warm-up steps
     precision = args.precision
@@ -398,9 +413,8 @@ def run_decomposed(args, rank, local_rank, world):
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    replicas.init("nccl", dev)
+    local_rank, dev = pick_device(local_rank)
+    replicas.init(dist_backend(), dev)
     K, W = args.steps, max(args.warmup, 20)
     p, phi, u, name = workload(args.config)
     if p.wall_flags & 4:

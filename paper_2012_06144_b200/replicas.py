@@ -40,7 +40,8 @@ def max_over_ranks(value: float, device=None) -> float:
     """Slowest rank's time: every multi-GPU number is reported as the max over ranks."""
     if not (dist.is_available() and dist.is_initialized()):
         return float(value)
-    t = torch.tensor([float(value)], dtype=torch.float64, device=device if device is not None else "cpu")
+    on_host = device is None or dist.get_backend() != "nccl"      # gloo reduces host tensors
+    t = torch.tensor([float(value)], dtype=torch.float64, device="cpu" if on_host else device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
 
