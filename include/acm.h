@@ -275,7 +275,10 @@ int acm_set_pdfs(acm_ctx*, const void* h, const void* g);
 
 /* End-to-end convenience with HOST buffers: copies phi (N) and u (3N) to the device,
  * acm_init, acm_step(n), then copies phi/u/p of the final state back (NULL = skipped) and
- * synchronises the stream.  Equivalent to the calls above plus the transfers. */
+ * synchronises the stream.  Equivalent to the calls above plus the transfers.  The result copies run on a private
+ * stream behind events, each as soon as its field is final: phi right after the last phase-field kernel (it travels
+ * while the last hydrodynamic kernel and the pressure export run), u after the last hydrodynamic kernel, p after its
+ * export; the context's stream waits for them before the call returns. */
 int acm_run_host(acm_ctx*, const void* phi_host, const void* u_host, int n,
                  void* phi_out_host, void* u_out_host, void* p_out_host);
 

@@ -76,6 +76,10 @@ struct acm_ctx {
     struct GraphEntry { unsigned key; cudaGraphExec_t exec; };
     std::vector<GraphEntry> graphs;  // one per buffer / storage-state parity the capture started from
     long long graph_replays;
+    // acm_run_host: the device-to-host copies of the results run on a private stream behind events, so that phi
+    // (final after the last phase-field kernel) already travels while the last hydrodynamic kernel runs
+    cudaStream_t io_stream;
+    cudaEvent_t io_ev[4];
 };
 
 // A graph holds an even number of steps: the buffer parity of the two-grid layout and the even/odd kernels of the
@@ -523,6 +527,8 @@ static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase,
     c->graph_mode = -1;
     c->cap_stream = nullptr;
     c->graph_replays = 0;
+    c->io_stream = nullptr;
+    for (auto& e : c->io_ev) e = nullptr;
     *out = c;
     return ACM_OK;
 }
@@ -721,6 +727,8 @@ void acm_destroy(acm_ctx* c)
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     graphs_clear(c);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+    if (c->io_stream) cudaStreamDestroy(c->io_stream);
+    for (cudaEvent_t e : c->io_ev) if (e) cudaEventDestroy(e);
     delete c;
 }
 
@@ -985,6 +993,25 @@ int acm_set_pdfs(acm_ctx* c, const void* h, const void* g)
     return rc;
 }
 
+// private stream and events of acm_run_host (created on first use)
+static bool io_ready(acm_ctx* c)
+{
+    if (c->io_stream) return true;
+    if (cudaStreamCreateWithFlags(&c->io_stream, cudaStreamNonBlocking) != cudaSuccess) { c->io_stream = nullptr; cudaGetLastError(); return false; }
+    for (auto& e : c->io_ev)
+        if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return false; }
+    return true;
+}
+
+// record `ev` on `from` and make `to` wait for it
+static int chain(acm_ctx* c, cudaEvent_t ev, cudaStream_t from, cudaStream_t to)
+{
+    cudaError_t e = cudaEventRecord(ev, from);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(to, ev, 0);
+    if (e != cudaSuccess) { c->sticky = ACM_ECUDA; return fail(ACM_ECUDA, "acm_run_host: %s", cudaGetErrorString(e)); }
+    return ACM_OK;
+}
+
 int acm_run_host(acm_ctx* c, const void* phi_host, const void* u_host, int n, void* phi_out_host, void* u_out_host,
                  void* p_out_host)
 {
@@ -997,18 +1024,50 @@ int acm_run_host(acm_ctx* c, const void* phi_host, const void* u_host, int n, vo
     int rc = copy_async(c, st, phi_host, fb, cudaMemcpyHostToDevice, "acm_run_host(h2d phi)");
     if (!rc) rc = copy_async(c, st + fb, u_host, 3 * fb, cudaMemcpyHostToDevice, "acm_run_host(h2d u)");
     if (!rc) rc = acm_init(c, st, st + fb);
-    if (!rc) rc = acm_step(c, n);
-    if (!rc && p_out_host) rc = acm_fields(c, nullptr, nullptr, st + 4 * fb);
-    if (!rc && phi_out_host) {
+    if (rc) return rc;
+    // Results go out on the private stream, each as soon as it is final: phi after the last phase-field kernel (under
+    // the last hydrodynamic kernel and the pressure export), u after the last hydrodynamic kernel, p after its export.
+    const bool overlap = n > 0 && io_ready(c);
+    const cudaStream_t main = c->stream, out = overlap ? c->io_stream : c->stream;
+    auto d2h = [&](void* dst, const void* src, size_t bytes, const char* what) {
+        cudaError_t e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, out);
+        if (e != cudaSuccess) { c->sticky = ACM_ECUDA; return fail(ACM_ECUDA, "%s: %s", what, cudaGetErrorString(e)); }
+        return (int)ACM_OK;
+    };
+    auto phi_out = [&]() {
+        if (!phi_out_host) return (int)ACM_OK;
         const char* src = c->ws + c->offC[c->curC];
         if (c->ref != 0.0) {      // un-shift phi into the staging area first (its phi/u slots are free after acm_init)
-            rc = copy_field_shifted(c, st, src, c->N, c->ref, "acm_run_host(phi)");
+            cudaError_t e = launch_shift_field<float>(out, (const float*)src, (float*)st, c->N, (float)c->ref);
+            int r = check_launch(c, "acm_run_host(phi)", e);
+            if (r) return r;
             src = st;
         }
-        if (!rc) rc = copy_async(c, phi_out_host, src, fb, cudaMemcpyDeviceToHost, "acm_run_host(d2h phi)");
+        return d2h(phi_out_host, src, fb, "acm_run_host(d2h phi)");
+    };
+    if (overlap) {
+        rc = acm_step(c, n - 1);
+        if (!rc) rc = c->precision == ACM_F64 ? launch_phase_step<double>(c) : launch_phase_step<float>(c);
+        if (!rc) rc = chain(c, c->io_ev[0], main, out);
+        if (!rc) rc = phi_out();
+        if (!rc) rc = c->precision == ACM_F64 ? launch_hydro_step<double>(c) : launch_hydro_step<float>(c);
+        if (!rc && u_out_host) {
+            rc = chain(c, c->io_ev[1], main, out);
+            if (!rc) rc = d2h(u_out_host, c->ws + c->offU[c->curU], 3 * fb, "acm_run_host(d2h u)");
+        }
+        if (!rc && p_out_host) {
+            rc = acm_fields(c, nullptr, nullptr, st + 4 * fb);
+            if (!rc) rc = chain(c, c->io_ev[2], main, out);
+            if (!rc) rc = d2h(p_out_host, st + 4 * fb, fb, "acm_run_host(d2h p)");
+        }
+        if (!rc) rc = chain(c, c->io_ev[3], out, main);      // the context's stream is complete when the copies are
+    } else {
+        rc = acm_step(c, n);
+        if (!rc && p_out_host) rc = acm_fields(c, nullptr, nullptr, st + 4 * fb);
+        if (!rc) rc = phi_out();
+        if (!rc && u_out_host) rc = d2h(u_out_host, c->ws + c->offU[c->curU], 3 * fb, "acm_run_host(d2h u)");
+        if (!rc && p_out_host) rc = d2h(p_out_host, st + 4 * fb, fb, "acm_run_host(d2h p)");
     }
-    if (!rc && u_out_host) rc = copy_async(c, u_out_host, c->ws + c->offU[c->curU], 3 * fb, cudaMemcpyDeviceToHost, "acm_run_host(d2h u)");
-    if (!rc && p_out_host) rc = copy_async(c, p_out_host, st + 4 * fb, fb, cudaMemcpyDeviceToHost, "acm_run_host(d2h p)");
     if (rc) return rc;
     cudaError_t e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) { c->sticky = ACM_ECUDA; return fail(ACM_ECUDA, "acm_run_host: %s", cudaGetErrorString(e)); }

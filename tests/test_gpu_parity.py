@@ -263,19 +263,32 @@ def test_uniform_state_exact():
     assert (ua.cpu().numpy() == 0).all()
 
 
-def test_run_host_matches_device_calls():
-    """acm_run_host (host buffers, transfers inside) == acm_init + acm_step + acm_fields."""
+@pytest.mark.parametrize("n,kw,outs", [(7, dict(), "cup"), (1, dict(), "cup"), (0, dict(), "cup"), (5, dict(precision="f32"), "cup"),
+                                       (3, dict(unfused=True), "cup"), (4, dict(inplace=True), "c"), (4, dict(), "p"), (4, dict(), "u")])
+def test_run_host_matches_device_calls(n, kw, outs):
+    """acm_run_host (host buffers, transfers inside; the result copies run on a private stream, phi already under the
+    last hydrodynamic kernel) == acm_init + acm_step + acm_fields, bit for bit; any output may be skipped."""
     p, phi, u = inputs.scaled_config3(24)
-    a = _acm(p)
+    dt = np.float32 if kw.get("precision") == "f32" else np.float64
+    phi, u = phi.astype(dt), u.astype(dt)
+    a = _acm(p, **kw)
     a.init(_dev(phi), _dev(u))
-    a.step(7)
+    a.step(n)
     pa, ua, pra = a.fields()
-    b = _acm(p)
+    b = _acm(p, **kw)
     ph = torch.from_numpy(phi).pin_memory()
     uh = torch.from_numpy(u).pin_memory()
-    po, uo, pro = torch.empty_like(ph).pin_memory(), torch.empty_like(uh).pin_memory(), torch.empty_like(ph).pin_memory()
-    b.run_host(ph, uh, 7, po, uo, pro)
-    assert (po == pa.cpu()).all() and (uo == ua.cpu()).all() and (pro == pra.cpu()).all()
+    po = torch.full_like(ph, -7.0).pin_memory() if "c" in outs else None
+    uo = torch.full_like(uh, -7.0).pin_memory() if "u" in outs else None
+    pro = torch.full_like(ph, -7.0).pin_memory() if "p" in outs else None
+    for _ in range(2):      # twice: the private stream and its events are reused
+        b.run_host(ph, uh, n, po, uo, pro)
+        assert po is None or (po == pa.cpu()).all()
+        assert uo is None or (uo == ua.cpu()).all()
+        assert pro is None or (pro == pra.cpu()).all()
+    # the context is in the state of the device calls afterwards
+    pb, ub, prb = b.fields()
+    assert torch.equal(pb, pa) and torch.equal(ub, ua) and torch.equal(prb, pra)
 
 
 def test_full_size_sampled_256():
