@@ -40,14 +40,15 @@ def test_two_replica_ranks_print_one_line():
     assert d["e2e"]["value"] > 0 and d["config"]["finite"]
 
 
-def test_two_slab_ranks_decomposed_halo_exchange_over_gloo_is_refused_or_runs():
-    """--decompose moves halo planes with torch.distributed P2P; over gloo those are host transfers of CUDA tensors,
-    which gloo does not offer -- the flow must fail loudly, not hang (the NCCL path needs two GPUs:
-    test_gpu_slab_ipc.py::test_two_gpus_over_nccl)."""
+def test_two_slab_ranks_over_gloo_fail_loudly():
+    """--decompose moves halo planes with torch.distributed P2P on CUDA tensors, which gloo does not offer: the run gets
+    through the slab set-up, initialisation and plan (the code both backends share) and must then fail loudly at the
+    first exchange -- no hang, no JSON line (the NCCL transport needs two GPUs: test_gpu_slab_ipc.py::test_two_gpus_over_nccl)."""
     env = dict(os.environ, ACM_DIST_BACKEND="gloo")
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr", "127.0.0.1",
            "--master-port", str(_free_port()), os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "2", "--warmup", "1",
            "--no-cpu-baseline", "--config", "1", "--decompose"]
     out = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT, env=env)
     lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
-    assert (out.returncode == 0 and len(lines) == 1) or (out.returncode != 0 and not lines)
+    assert out.returncode != 0 and not lines
+    assert "refresh_halos" in out.stderr and "batch_isend_irecv" in out.stderr      # it got as far as the first exchange
