@@ -102,8 +102,19 @@ int acm_create(acm_ctx** out, int nx, int ny, int nz, int stencil_phase, int ste
  *   ACM_OPT_BULK_ONE  the other reading of "we relax the second order moments with s_nu ... all other moments are
  *                     relaxed by one" (A4/A26): only the five deviatoric second-order
  *                     moments relax with s_nu, their trace (the bulk moment) with 1.  Same shear viscosity,
- *                     bulk viscosity 1/9 instead of 2 nu/3.  Not with ACM_OPT_UNFUSED or slabs (ACM_EINVAL). */
-enum { ACM_OPT_INPLACE = 1, ACM_OPT_PHASE_SRT = 2, ACM_OPT_UNFUSED = 4, ACM_OPT_BULK_ONE = 8, ACM_OPT_ALL = 15 };
+ *                     bulk viscosity 1/9 instead of 2 nu/3.  Not with ACM_OPT_UNFUSED or slabs (ACM_EINVAL).
+ *   ACM_OPT_MOMENTS   moment representation of the state (beyond the paper, last paragraph).  The paper's
+ *                     collisions relax every moment of h beyond the first order and of g beyond the second order
+ *                     with rate 1, so the post-collision populations of a cell are
+ *                     w_i [A + e_i.b + e_i e_i : T] with 4 (h: A, b; T = 4.5 phi u u^T follows from phi and u) and
+ *                     10 (g: A, b, T) numbers.  The workspace then holds those instead of Q_h + Q_g populations and the
+ *                     pull of the next step rebuilds the one population each neighbour contributes; u is
+ *                     double-buffered.  Same time step, same results up to rounding (same bars against the oracle);
+ *                     128 + 216 B of traffic per cell and step for every lattice instead of 8 (2 Q_h + 5) +
+ *                     8 (2 Q_g + 7).  ACM_F64 only; not with ACM_OPT_INPLACE / ACM_OPT_UNFUSED / ACM_OPT_PHASE_SRT
+ *                     (SRT keeps every moment) or slabs (ACM_EINVAL); acm_set_pdfs returns ACM_EINVAL (arbitrary
+ *                     populations have no such representation), acm_get_pdfs rebuilds the populations. */
+enum { ACM_OPT_INPLACE = 1, ACM_OPT_PHASE_SRT = 2, ACM_OPT_UNFUSED = 4, ACM_OPT_BULK_ONE = 8, ACM_OPT_MOMENTS = 16, ACM_OPT_ALL = 31 };
 size_t acm_workspace_bytes_opt(int nx, int ny, int nz, int stencil_phase, int stencil_hydro, int precision,
                                unsigned options);
 /* acm_create with options; acm_create(...) == acm_create_opt(..., options = 0, ...). */

@@ -16,7 +16,7 @@ from . import build as _build
 ACM_OK, ACM_EINVAL, ACM_ESTATE, ACM_ECUDA, ACM_EUNSTABLE = 0, 1, 2, 3, 4
 ACM_F64, ACM_F32 = 0, 1
 ACM_WALL_X, ACM_WALL_Y, ACM_WALL_Z = 1, 2, 4
-ACM_OPT_INPLACE, ACM_OPT_PHASE_SRT, ACM_OPT_UNFUSED, ACM_OPT_BULK_ONE = 1, 2, 4, 8
+ACM_OPT_INPLACE, ACM_OPT_PHASE_SRT, ACM_OPT_UNFUSED, ACM_OPT_BULK_ONE, ACM_OPT_MOMENTS = 1, 2, 4, 8, 16
 
 EXPORTS = ["acm_workspace_bytes", "acm_workspace_bytes_opt", "acm_create", "acm_create_opt", "acm_init", "acm_step", "acm_fields", "acm_phi_mass", "acm_get_pdfs",
            "acm_set_pdfs", "acm_run_host", "acm_set_reference_phase", "acm_bubble_diag", "acm_bubble_sums", "acm_slab_range", "acm_workspace_bytes_slab", "acm_create_slab", "acm_slab_info",
@@ -129,7 +129,7 @@ class ACM:
     def __init__(self, nx, ny, nz, stencil_phase=15, stencil_hydro=19, rho_H=1.0, rho_L=1e-3, sigma=1e-4, xi=5.0,
                  M=0.02, nu_H=1 / 60, nu_L=1 / 60, gravity=(0.0, 0.0, 0.0), wall_flags=0, precision="f64",
                  device="cuda:0", stream=None, inplace=False, phase_srt=False, unfused=False, bulk_one=False, subiter=1,
-                 guard_bytes=0):
+                 guard_bytes=0, moments=False):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2012_06144_b200 needs a CUDA device (no CPU fallback)")
         self._lib = load()
@@ -142,7 +142,7 @@ class ACM:
         self.dtype = torch.float64 if precision == "f64" else torch.float32
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self.options = ((ACM_OPT_INPLACE if inplace else 0) | (ACM_OPT_PHASE_SRT if phase_srt else 0) | (ACM_OPT_UNFUSED if unfused else 0)
-                        | (ACM_OPT_BULK_ONE if bulk_one else 0))
+                        | (ACM_OPT_BULK_ONE if bulk_one else 0) | (ACM_OPT_MOMENTS if moments else 0))
         nbytes = self._lib.acm_workspace_bytes_opt(self.nx, self.ny, self.nz, self.Qh, self.Qg, self.precision,
                                                    self.options)
         if nbytes == 0:

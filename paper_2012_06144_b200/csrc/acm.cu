@@ -10,11 +10,14 @@
 //   C[2][N]      phi (double-buffered: the phase kernel reads a stencil of the old phi and writes new)
 //   U[3][N]      velocity, in place
 // With ACM_OPT_INPLACE there is one H and one G array (AA pattern, see common.cuh).
+// With ACM_OPT_MOMENTS the H region holds M[2][4][N] and the G region K[2][10][N] (the coefficients of the
+// post-collision state, moment_impl.cuh) and U is double-buffered.
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <type_traits>
 #include <vector>
 
 #include "kernels.h"
@@ -54,6 +57,7 @@ struct acm_ctx {
     // carved workspace (byte offsets)
     size_t offH[2], offG[2], offC[2], offU[2], offStage, offRed;
     int curH, curG, curC, curU;       // which buffer holds the current state
+    int uH;                           // ACM_OPT_MOMENTS: the velocity buffer the current coefficients of h* were built with
     unsigned options;           // ACM_OPT_*
     int stH, stG;               // storage state of the current H / G buffer (ST_POST | ST_IN | ST_SWAP)
     bool initialised;
@@ -91,6 +95,8 @@ static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
 static bool valid_stencil(int q) { return q == 9 || q == 15 || q == 19 || q == 27; }
 
+constexpr size_t MOM_H = 4, MOM_G = 10;      // planes of the coefficient arrays M (A, b) and K (A, b, T)
+
 struct Layout {
     size_t offH[2], offG[2], offC[2], offU[2], offStage, offRed, total;
 };
@@ -99,6 +105,8 @@ static bool make_layout(int nx, int ny, int nz, int Qh, int Qg, int precision, u
 {
     if (options & ~(unsigned)ACM_OPT_ALL) return false;
     if ((options & ACM_OPT_UNFUSED) && (options & ACM_OPT_INPLACE)) return false;   // Algorithm 1 is a two-grid scheme
+    // moment representation: two-grid fused kernels, MRT phase-field collision (SRT keeps every moment), fp64
+    if ((options & ACM_OPT_MOMENTS) && ((options & (ACM_OPT_INPLACE | ACM_OPT_UNFUSED | ACM_OPT_PHASE_SRT)) || precision != ACM_F64)) return false;
     const int grids = (options & ACM_OPT_INPLACE) ? 1 : 2;
     if (nx <= 0 || ny <= 0 || nz <= 0 || !valid_stencil(Qh) || !valid_stencil(Qg)) return false;
     if ((Qh == 9) != (Qg == 9)) return false;      // the two-dimensional instance uses D2Q9 for both LB steps
@@ -107,12 +115,15 @@ static bool make_layout(int nx, int ny, int nz, int Qh, int Qg, int precision, u
     if (cells >= 2147483648.0) return false;
     const size_t N = (size_t)nx * ny * nz, e = precision == ACM_F64 ? 8 : 4;
     size_t o = 0;
-    for (int b = 0; b < grids; ++b) { L->offH[b] = o; o = align256(o + (size_t)Qh * N * e); }
-    for (int b = 0; b < grids; ++b) { L->offG[b] = o; o = align256(o + (size_t)Qg * N * e); }
+    // planes per population set: the populations, or the coefficients of the moment representation (A, b / A, b, T)
+    const bool mom = (options & ACM_OPT_MOMENTS) != 0;
+    const size_t Sh = mom ? MOM_H : (size_t)Qh, Sg = mom ? MOM_G : (size_t)Qg;
+    for (int b = 0; b < grids; ++b) { L->offH[b] = o; o = align256(o + Sh * N * e); }
+    for (int b = 0; b < grids; ++b) { L->offG[b] = o; o = align256(o + Sg * N * e); }
     if (grids == 1) { L->offH[1] = L->offH[0]; L->offG[1] = L->offG[0]; }
     for (int b = 0; b < 2; ++b) { L->offC[b] = o; o = align256(o + N * e); }
     L->offU[0] = L->offU[1] = o; o = align256(o + 3 * N * e);
-    if (options & ACM_OPT_UNFUSED) { L->offU[1] = o; o = align256(o + 3 * N * e); }   // u double-buffered (unfused_impl.cuh)
+    if (options & (ACM_OPT_UNFUSED | ACM_OPT_MOMENTS)) { L->offU[1] = o; o = align256(o + 3 * N * e); }   // u double-buffered (unfused_impl.cuh, moment_impl.cuh)
     L->offStage = o; o = align256(o + 5 * N * e);
     L->offRed = o; o = align256(o + (size_t)DIAG_WIDTH * (RED_BLOCKS + 1) * sizeof(double));
     L->total = o;
@@ -170,11 +181,19 @@ static int init_t(acm_ctx* c, const void* phi, const void* u)
 {
     const bool inplace = (c->options & ACM_OPT_INPLACE) != 0;
     T *H = wsp<T>(c, c->offH[0]), *G = wsp<T>(c, c->offG[0]), *C = wsp<T>(c, c->offC[0]), *U = wsp<T>(c, c->offU[0]);
+    if (c->options & ACM_OPT_MOMENTS) {
+        if constexpr (std::is_same<T, double>::value) {
+            cudaError_t e = launch_init_mom<T>(aux_launch(c), (const T*)phi, (const T*)u, H, G, C, U, wsp<T>(c, c->offU[1]), geom_of(c), c->N);
+            c->stH = ST_POST; c->stG = ST_IN;      // g: the cell's own incoming populations until the first hydrodynamic step
+            c->curH = c->curG = c->curC = c->curU = c->uH = 0;
+            return check_launch(c, "init_mom_kernel", e);
+        } else return fail(ACM_EINVAL, "acm_init: ACM_OPT_MOMENTS is fp64 only");
+    }
     cudaError_t e = launch_init<T>(c->Qh, c->Qg, inplace, aux_launch(c), (const T*)phi, (const T*)u, H, G, C, U,
                                    geom_of(c), c->N, (T)c->ref);
     if (inplace) { c->stH = ST_SWAP; c->stG = ST_IN; }
     else c->stH = c->stG = ST_POST;
-    c->curH = c->curG = c->curC = c->curU = 0;
+    c->curH = c->curG = c->curC = c->curU = c->uH = 0;
     return check_launch(c, "init_kernel", e);
 }
 
@@ -197,6 +216,21 @@ template <typename T>
 static int launch_phase_range(acm_ctx* c, int z0, int z1)
 {
     if (z1 <= z0) return ACM_OK;
+    if (c->options & ACM_OPT_MOMENTS) {
+        if constexpr (std::is_same<T, double>::value) {
+            MomPhaseArgs<T> a;
+            a.Msrc = wsp<T>(c, c->offH[c->curH]); a.Mdst = wsp<T>(c, c->offH[c->curH ^ 1]);
+            a.Csrc = wsp<T>(c, c->offC[c->curC]); a.Cdst = wsp<T>(c, c->offC[c->curC ^ 1]);
+            a.Uold = wsp<T>(c, c->offU[c->uH]); a.U = wsp<T>(c, c->offU[c->curU]);
+            a.g = geom_of(c, lb_linear(c, 1), z0, z1);
+            a.N = (unsigned)c->N;
+            a.one_minus_omega = (T)(1.0 - 1.0 / (3.0 * c->M + 0.5));
+            a.inv_xi = (T)(1.0 / c->xi);
+            cudaError_t e = launch_phase_mom<T>(c->Qh, c->walls != 0, lb_launch(c, z1 - z0, 1), a);
+            c->phase_planes += z1 - z0;
+            return check_launch(c, "phase_mom_kernel", e);
+        } else return fail(ACM_EINVAL, "ACM_OPT_MOMENTS is fp64 only");
+    }
     PhaseArgs<T> a;
     a.Hsrc = wsp<T>(c, c->offH[c->curH]); a.Hdst = wsp<T>(c, c->offH[c->curH ^ 1]);
     a.Csrc = wsp<T>(c, c->offC[c->curC]); a.Cdst = wsp<T>(c, c->offC[c->curC ^ 1]);
@@ -224,6 +258,7 @@ static void commit_phase(acm_ctx* c)
 {
     c->phase_planes = 0;
     c->curH ^= 1; c->curC ^= 1;
+    c->uH = c->curU;      // the velocity this phase-field step collided with
     c->stH = next_state(c->stH);
 }
 
@@ -248,6 +283,18 @@ static int launch_hydro_range(acm_ctx* c, int z0, int z1)
     a.subiter = c->subiter;
     a.Gpeer = peers_at<T>(c, c->offG[c->curG]);
     a.Cpeer = peers_at<T>(c, c->offC[c->curC]);
+    if (c->options & ACM_OPT_MOMENTS) {
+        if constexpr (std::is_same<T, double>::value) {
+            MomHydroArgs<T> ma;
+            ma.h = a;
+            ma.h.g = geom_of(c, lb_linear(c, 1), z0, z1);
+            ma.Ksrc = wsp<T>(c, c->offG[c->curG]); ma.Kdst = wsp<T>(c, c->offG[c->curG ^ 1]);
+            ma.Uin = wsp<T>(c, c->offU[c->curU]); ma.Uout = wsp<T>(c, c->offU[c->curU ^ 1]);
+            cudaError_t e = launch_hydro_mom<T>(c->Qg, c->walls != 0, c->stG == ST_IN, lb_launch(c, z1 - z0, 1), ma);
+            c->hydro_planes += z1 - z0;
+            return check_launch(c, "hydro_mom_kernel", e);
+        } else return fail(ACM_EINVAL, "ACM_OPT_MOMENTS is fp64 only");
+    }
     const Launch l = lb_launch(c, z1 - z0, cpt);
     const bool unfused = (c->options & ACM_OPT_UNFUSED) != 0;
     cudaError_t e = unfused ? launch_unfused_hydro<T>(c->Qg, c->walls != 0, l, a, wsp<T>(c, c->offU[c->curU]), wsp<T>(c, c->offU[c->curU ^ 1]))
@@ -261,9 +308,9 @@ static void commit_hydro(acm_ctx* c)
 {
     c->hydro_planes = 0;
     c->steps_done += 1;
-    if (c->options & ACM_OPT_UNFUSED) c->curU ^= 1;
+    if (c->options & (ACM_OPT_UNFUSED | ACM_OPT_MOMENTS)) c->curU ^= 1;
     c->curG ^= 1;
-    c->stG = next_state(c->stG);
+    c->stG = (c->options & ACM_OPT_MOMENTS) ? ST_POST : next_state(c->stG);
 }
 
 template <typename T>
@@ -307,7 +354,7 @@ static void graphs_clear(acm_ctx* c)
 
 static unsigned graph_key(const acm_ctx* c)
 {
-    return (unsigned)c->curH | (unsigned)c->curG << 1 | (unsigned)c->curC << 2 | (unsigned)c->curU << 3 | (unsigned)c->stH << 4 | (unsigned)c->stG << 6;
+    return (unsigned)c->curH | (unsigned)c->curG << 1 | (unsigned)c->curC << 2 | (unsigned)c->curU << 3 | (unsigned)c->stH << 4 | (unsigned)c->stG << 6 | (unsigned)c->uH << 8;
 }
 
 static bool graph_wanted(const acm_ctx* c)
@@ -328,6 +375,7 @@ static cudaGraphExec_t graph_for_state(acm_ctx* c)
     if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return nullptr; }
     const cudaStream_t user = c->stream;
     const long long launches = c->launches, steps_done = c->steps_done;
+    const int stG = c->stG, uH = c->uH;      // moment representation: these two do not come back after an even count
     c->stream = c->cap_stream;
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
@@ -341,6 +389,7 @@ static cudaGraphExec_t graph_for_state(acm_ctx* c)
     c->stream = user;
     c->launches = launches;
     c->steps_done = steps_done;
+    c->stG = stG; c->uH = uH;
     if (!ok) {
         cudaGetLastError();
         c->sticky = ACM_OK;          // a failed capture is not a failed launch: fall back to plain launches
@@ -385,6 +434,7 @@ static int step_t(acm_ctx* c, int n)
             c->steps_done += GRAPH_STEPS;
             c->graph_replays += 1;
             done += GRAPH_STEPS;
+            if (c->options & ACM_OPT_MOMENTS) { c->stG = ST_POST; c->uH = c->curU ^ 1; }      // the state any completed step leaves
         }
     }
     return plain_steps<T>(c, n - done);
@@ -393,6 +443,13 @@ static int step_t(acm_ctx* c, int n)
 template <typename T>
 static int export_g_t(acm_ctx* c, void* g, void* p)      // incoming convention (+ pressure)
 {
+    if (c->options & ACM_OPT_MOMENTS) {
+        if constexpr (std::is_same<T, double>::value) {
+            cudaError_t e = launch_export_g_mom<T>(c->Qg, c->stG == ST_IN, aux_launch(c), wsp<T>(c, c->offG[c->curG]), wsp<T>(c, c->offC[c->curC]),
+                                                   (T*)g, (T*)p, geom_of(c), c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L));
+            return check_launch(c, "export_g_mom_kernel", e);
+        } else return fail(ACM_EINVAL, "ACM_OPT_MOMENTS is fp64 only");
+    }
     cudaError_t e = launch_export<T>(c->Qg, c->stG, false, aux_launch(c), wsp<T>(c, c->offG[c->curG]), wsp<T>(c, c->offC[c->curC]),
                                      (T*)g, (T*)p, geom_of(c), c->N, (T)(c->rho_L + c->ref * (c->rho_H - c->rho_L)), (T)(c->rho_H - c->rho_L), (T)0);
     return check_launch(c, "export_kernel", e);
@@ -401,6 +458,13 @@ static int export_g_t(acm_ctx* c, void* g, void* p)      // incoming convention 
 template <typename T>
 static int export_h_t(acm_ctx* c, void* h)               // post-collision convention
 {
+    if (c->options & ACM_OPT_MOMENTS) {
+        if constexpr (std::is_same<T, double>::value) {
+            cudaError_t e = launch_export_h_mom<T>(c->Qh, aux_launch(c), wsp<T>(c, c->offH[c->curH]), wsp<T>(c, c->offC[c->curC]),
+                                                   wsp<T>(c, c->offU[c->uH]), (T*)h, geom_of(c), c->N);
+            return check_launch(c, "export_h_mom_kernel", e);
+        } else return fail(ACM_EINVAL, "ACM_OPT_MOMENTS is fp64 only");
+    }
     cudaError_t e = launch_export<T>(c->Qh, c->stH, true, aux_launch(c), wsp<T>(c, c->offH[c->curH]), wsp<T>(c, c->offC[c->curC]),
                                      (T*)h, (T*)nullptr, geom_of(c), c->N, (T)c->rho_L, (T)(c->rho_H - c->rho_L), (T)c->ref);
     return check_launch(c, "export_kernel", e);
@@ -454,7 +518,7 @@ static int copy_field_shifted(acm_ctx* c, void* dst, const void* src, size_t n, 
 // 256 fp32 cells (128 pairs) along x; single-cell fp32 falls back to 128 when nx is not a multiple of 256.
 static void default_cells_per_thread(acm_ctx* c)
 {
-    const bool can_pair = c->nx % 2 == 0 && !(c->options & ACM_OPT_UNFUSED);
+    const bool can_pair = c->nx % 2 == 0 && !(c->options & (ACM_OPT_UNFUSED | ACM_OPT_MOMENTS));
     const bool f32 = c->precision == ACM_F32;
     c->cpt_phase = (can_pair && (f32 || c->Qh <= 19)) ? 2 : 1;
     c->cpt_hydro = (can_pair && (f32 || c->Qg == 15 || c->Qg == 19)) ? 2 : 1;
@@ -472,8 +536,8 @@ static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase,
     if ((options & ACM_OPT_BULK_ONE) && (options & ACM_OPT_UNFUSED))
         return fail(ACM_EINVAL, "acm_create: ACM_OPT_BULK_ONE is not available with ACM_OPT_UNFUSED");
     if (slab) {
-        if (options & (ACM_OPT_INPLACE | ACM_OPT_UNFUSED | ACM_OPT_BULK_ONE))
-            return fail(ACM_EINVAL, "acm_create_slab: ACM_OPT_INPLACE / ACM_OPT_UNFUSED / ACM_OPT_BULK_ONE are not available for slabs");
+        if (options & (ACM_OPT_INPLACE | ACM_OPT_UNFUSED | ACM_OPT_BULK_ONE | ACM_OPT_MOMENTS))
+            return fail(ACM_EINVAL, "acm_create_slab: ACM_OPT_INPLACE / ACM_OPT_UNFUSED / ACM_OPT_BULK_ONE / ACM_OPT_MOMENTS are not available for slabs");
         if (nz > 0) nz += 2;      // ghost planes below and above
     }
     if (!out) return fail(ACM_EINVAL, "acm_create: out is NULL");
@@ -682,6 +746,7 @@ int acm_phase_launch(acm_ctx* c, int z0, int z1)
     ACM_CHECK_CTX(c);
     if (!c->initialised) return fail(ACM_ESTATE, "acm_phase_launch: call acm_init first");
     if (z0 < 0 || z1 > c->nzl || z0 > z1) return fail(ACM_EINVAL, "acm_phase_launch: need 0 <= z0 <= z1 <= owned planes");
+    if (c->options & ACM_OPT_MOMENTS) return fail(ACM_ESTATE, "acm_phase_launch: not available with ACM_OPT_MOMENTS (use acm_step)");
     if (c->phase_planes + (z1 - z0) > c->nzl) return fail(ACM_ESTATE, "acm_phase_launch: more planes than the slab owns since the last acm_phase_commit");
     if (c->hydro_planes) return fail(ACM_ESTATE, "acm_phase_launch: the hydrodynamic step is not committed");
     return c->precision == ACM_F64 ? launch_phase_range<double>(c, z0, z1) : launch_phase_range<float>(c, z0, z1);
@@ -701,6 +766,7 @@ int acm_hydro_launch(acm_ctx* c, int z0, int z1)
     ACM_CHECK_CTX(c);
     if (!c->initialised) return fail(ACM_ESTATE, "acm_hydro_launch: call acm_init first");
     if (z0 < 0 || z1 > c->nzl || z0 > z1) return fail(ACM_EINVAL, "acm_hydro_launch: need 0 <= z0 <= z1 <= owned planes");
+    if (c->options & ACM_OPT_MOMENTS) return fail(ACM_ESTATE, "acm_hydro_launch: not available with ACM_OPT_MOMENTS (use acm_step)");
     if (c->hydro_planes + (z1 - z0) > c->nzl) return fail(ACM_ESTATE, "acm_hydro_launch: more planes than the slab owns since the last acm_hydro_commit");
     if (c->phase_planes) return fail(ACM_ESTATE, "acm_hydro_launch: the phase-field step is not committed");
     return c->precision == ACM_F64 ? launch_hydro_range<double>(c, z0, z1) : launch_hydro_range<float>(c, z0, z1);
@@ -781,7 +847,7 @@ int acm_set_cells_per_thread(acm_ctx* c, int phase, int hydro)
 {
     ACM_CHECK_CTX(c);
     if (phase < 0 || phase > 2 || hydro < 0 || hydro > 2) return fail(ACM_EINVAL, "acm_set_cells_per_thread: 0 (default), 1 or 2");
-    if ((phase == 2 || hydro == 2) && (c->nx % 2 != 0 || (c->options & ACM_OPT_UNFUSED)))
+    if ((phase == 2 || hydro == 2) && (c->nx % 2 != 0 || (c->options & (ACM_OPT_UNFUSED | ACM_OPT_MOMENTS))))
         return fail(ACM_EINVAL, "acm_set_cells_per_thread: two cells per thread need an even nx and the fused kernels");
     if (c->phase_planes || c->hydro_planes) return fail(ACM_ESTATE, "acm_set_cells_per_thread: a step is partly launched (commit it first)");
     const dim3 block = c->block;
@@ -977,6 +1043,8 @@ int acm_set_pdfs(acm_ctx* c, const void* h, const void* g)
 {
     ACM_CHECK_CTX(c);
     if (!c->initialised) return fail(ACM_ESTATE, "acm_set_pdfs: call acm_init first");
+    if (c->options & ACM_OPT_MOMENTS)
+        return fail(ACM_EINVAL, "acm_set_pdfs: not available with ACM_OPT_MOMENTS (arbitrary populations have no moment representation)");
     int rc = ACM_OK;
     const bool inplace = (c->options & ACM_OPT_INPLACE) != 0;
     if (h) {

@@ -286,4 +286,23 @@ struct HydroArgs {
     Peers<T> Gpeer, Cpeer;   // peer mode of a slab (else unused)
 };
 
+// argument blocks of the kernels in moment representation (ACM_OPT_MOMENTS, moment_impl.cuh)
+template <typename T>
+struct MomPhaseArgs {
+    const T* Msrc; T* Mdst;      // [4][N]: A, b of h*
+    const T* Csrc; T* Cdst;      // phi
+    const T* Uold;               // velocity the collision that wrote Msrc used (read at the neighbours)
+    const T* U;                  // current velocity (read at the cell)
+    Geom g;
+    unsigned N;
+    T one_minus_omega, inv_xi;
+};
+
+template <typename T>
+struct MomHydroArgs {
+    HydroArgs<T> h;              // constants, new phi (h.C), geometry; h.Gsrc / h.Gdst / h.U are not used
+    const T* Ksrc; T* Kdst;      // [10][N]: A, b, T of g*
+    const T* Uin; T* Uout;       // velocity of the previous step (read at the cell) / of this step
+};
+
 }  // namespace acm

@@ -28,6 +28,15 @@ template <typename T> cudaError_t launch_hydro2(int Q, bool walls, int state, co
 template <typename T> cudaError_t launch_unfused_phase(int Q, bool walls, int collision, const Launch& l, const PhaseArgs<T>& a);
 template <typename T> cudaError_t launch_unfused_hydro(int Q, bool walls, const Launch& l, const HydroArgs<T>& a, const T* Uold, T* Unew);
 
+// The two fused kernels in moment representation (ACM_OPT_MOMENTS; moment_impl.cuh), their initialiser and exports.
+// local: the coefficient array of g holds the cell's own incoming populations (state right after acm_init).
+template <typename T> cudaError_t launch_phase_mom(int Q, bool walls, const Launch& l, const MomPhaseArgs<T>& a);
+template <typename T> cudaError_t launch_hydro_mom(int Q, bool walls, bool local, const Launch& l, const MomHydroArgs<T>& a);
+template <typename T> cudaError_t launch_init_mom(const Launch& l, const T* phi, const T* u, T* M, T* K, T* C, T* U0, T* U1, Geom g, size_t N);
+template <typename T> cudaError_t launch_export_h_mom(int Q, const Launch& l, const T* M, const T* C, const T* Uo, T* out, Geom g, size_t N);
+template <typename T>
+cudaError_t launch_export_g_mom(int Q, bool local, const Launch& l, const T* K, const T* C, T* out, T* p, Geom g, size_t N, T rho_L, T drho);
+
 // Equilibrium initialiser.
 template <typename T>
 cudaError_t launch_init(int Qh, int Qg, bool inplace, const Launch& l, const T* phi, const T* u, T* H, T* G, T* C, T* U, Geom g, size_t N, T ref);

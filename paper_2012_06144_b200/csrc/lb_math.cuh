@@ -152,10 +152,17 @@ __device__ __forceinline__ HydroCell<T> hydro_velocity(const Moments<Q, T, true>
     return HydroCell<T>{ux, uy, uz, hx, hy, hz, s_nu, Sxx, Syy, Szz};
 }
 
-// Hydrodynamic collision at one cell (eqs. 10-12, 25 in closed form): emits the
-// post-collision populations through store(ic, value).
-template <typename T, int Q, int HVAR = 0, typename S, typename Store>
-__device__ __forceinline__ void hydro_collide(const Moments<Q, T, true>& m, const HydroCell<T>& hc, const HydroArgs<S>& a, Store&& store)
+// Coefficients of a closed-form collision result  f*_i = w_i [A + e_i.b + e_i e_i : T]  (T symmetric).  Because all
+// moments beyond the first (phase field) / second (hydrodynamics) order relax with rate 1, these ten numbers ARE the
+// post-collision state of a cell: the moment representation of moment_impl.cuh stores them instead of the populations.
+template <typename T>
+struct Coeffs {
+    T A, bx, by, bz, Txx, Tyy, Tzz, Txy, Txz, Tyz;
+};
+
+// Hydrodynamic collision at one cell (eqs. 10-12, 25 in closed form): the coefficients of g*.
+template <typename T, int Q, int HVAR = 0, typename S>
+__device__ __forceinline__ Coeffs<T> hydro_coeffs(const Moments<Q, T, true>& m, const HydroCell<T>& hc, const HydroArgs<S>& a)
 {
     const T pstar = m.m0;
     const T ux = hc.ux, uy = hc.uy, uz = hc.uz, hx = hc.hx, hy = hc.hy, hz = hc.hz, s_nu = hc.s_nu;
@@ -181,7 +188,15 @@ __device__ __forceinline__ void hydro_collide(const Moments<Q, T, true>& m, cons
         }
     }
     const T bx = T(3) * (ux + hx), by = T(3) * (uy + hy), bz = T(3) * (uz + hz);
-    emit_populations<Q, T>(A, bx, by, bz, Txx, Tyy, Tzz, Txy, Txz, Tyz, store);
+    return Coeffs<T>{A, bx, by, bz, Txx, Tyy, Tzz, Txy, Txz, Tyz};
+}
+
+// ... and the populations they stand for, emitted through store(ic, value).
+template <typename T, int Q, int HVAR = 0, typename S, typename Store>
+__device__ __forceinline__ void hydro_collide(const Moments<Q, T, true>& m, const HydroCell<T>& hc, const HydroArgs<S>& a, Store&& store)
+{
+    const Coeffs<T> k = hydro_coeffs<T, Q, HVAR>(m, hc, a);
+    emit_populations<Q, T>(k.A, k.bx, k.by, k.bz, k.Txx, k.Tyy, k.Tzz, k.Txy, k.Txz, k.Tyz, store);
 }
 
 }  // namespace acm
