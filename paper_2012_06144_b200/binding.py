@@ -20,7 +20,7 @@ ACM_OPT_INPLACE, ACM_OPT_PHASE_SRT, ACM_OPT_UNFUSED, ACM_OPT_BULK_ONE, ACM_OPT_M
 
 EXPORTS = ["acm_workspace_bytes", "acm_workspace_bytes_opt", "acm_create", "acm_create_opt", "acm_init", "acm_step", "acm_fields", "acm_phi_mass", "acm_get_pdfs",
            "acm_set_pdfs", "acm_run_host", "acm_set_reference_phase", "acm_bubble_diag", "acm_bubble_sums", "acm_slab_range", "acm_workspace_bytes_slab", "acm_create_slab", "acm_slab_info",
-           "acm_halo_plan", "acm_set_peers", "acm_state_signature", "acm_phase_launch", "acm_phase_commit", "acm_hydro_launch", "acm_hydro_commit", "acm_bubble_params", "acm_drag_lbm", "acm_drag_exp", "acm_set_block", "acm_set_cells_per_thread", "acm_set_subiter", "acm_set_graph", "acm_graph_replays", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
+           "acm_halo_plan", "acm_set_peers", "acm_state_signature", "acm_phase_launch", "acm_phase_commit", "acm_hydro_launch", "acm_hydro_commit", "acm_bubble_params", "acm_drag_lbm", "acm_drag_exp", "acm_set_block", "acm_set_cells_per_thread", "acm_set_subiter", "acm_set_moment_kernels", "acm_set_graph", "acm_graph_replays", "acm_profile", "acm_profile_read", "acm_launch_count", "acm_destroy", "acm_last_error"]
 
 _lib = None
 
@@ -85,6 +85,7 @@ def load(build_if_missing: bool = True):
     lib.acm_set_subiter.argtypes = [vp, i32]
     lib.acm_set_cells_per_thread.argtypes = [vp, i32, i32]
     lib.acm_set_graph.argtypes = [vp, i32]
+    lib.acm_set_moment_kernels.argtypes = [vp, i32, i32]
     lib.acm_graph_replays.argtypes = [vp]
     lib.acm_graph_replays.restype = C.c_longlong
     lib.acm_profile.argtypes = [vp, i32]
@@ -227,6 +228,9 @@ class ACM:
     def set_subiter(self, sweeps):
         """sweeps of the fixed point of eq. 22 (1 = single evaluation of F_mu with the previous velocity)"""
         self._call(self._lib.acm_set_subiter, int(sweeps))
+
+    def set_moment_kernels(self, mode=-1, zchunk=0):
+        self._call(self._lib.acm_set_moment_kernels, int(mode), int(zchunk))
 
     def set_graph(self, mode):
         """CUDA graphs of 16 steps in acm_step: -1 automatic (small grids), 0 never, 1 always"""

@@ -58,6 +58,8 @@ struct acm_ctx {
     size_t offH[2], offG[2], offC[2], offU[2], offStage, offRed;
     int curH, curG, curC, curU;       // which buffer holds the current state
     int uH;                           // ACM_OPT_MOMENTS: the velocity buffer the current coefficients of h* were built with
+    int mom_mode, mom_zchunk;         // ACM_OPT_MOMENTS: -1 automatic | 0 direct kernels | 1 marching kernels; planes per block (0 = automatic)
+    int sm_count;
     unsigned options;           // ACM_OPT_*
     int stH, stG;               // storage state of the current H / G buffer (ST_POST | ST_IN | ST_SWAP)
     bool initialised;
@@ -171,6 +173,29 @@ static Launch launch_over(const acm_ctx* c, dim3 b, bool linear, int nplanes, in
 
 static Launch lb_launch(const acm_ctx* c, int nplanes, int cpt) { return launch_over(c, c->block, lb_linear(c, cpt), nplanes, cpt); }
 
+// Moment representation: the marching kernels (shared-memory window, moment_impl.cuh) for grids that fill the GPU, the
+// direct kernels otherwise; planes per block chosen such that the blocks fill whole waves of 2 blocks per SM, counting
+// the two extra planes a chunk reads.
+static bool mom_march(const acm_ctx* c)
+{
+    if (c->mom_mode >= 0) return c->mom_mode == 1;
+    return c->Qh != 9 && (size_t)c->nx * c->ny * c->nzl >= ((size_t)1 << 21);
+}
+
+static int mom_zchunk(const acm_ctx* c, int planes)
+{
+    if (c->mom_zchunk > 0) return c->mom_zchunk < planes ? c->mom_zchunk : planes;
+    const long long tiles = (long long)((c->nx + 31) / 32) * ((c->ny + 7) / 8), slots = 2LL * (c->sm_count > 0 ? c->sm_count : 148);
+    int best = planes;
+    double best_eff = -1.0;
+    for (int zc = planes < 8 ? planes : 8; zc <= planes; ++zc) {
+        const long long blocks = tiles * ((planes + zc - 1) / zc), waves = (blocks + slots - 1) / slots;
+        const double eff = (double)blocks / (double)(waves * slots) * zc / (zc + 1.0);
+        if (eff > best_eff + 1e-9) { best_eff = eff; best = zc; }
+    }
+    return best;
+}
+
 template <typename T> static T* wsp(acm_ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }
 
 // ---- typed implementations -----------------------------------------------------------------
@@ -226,9 +251,12 @@ static int launch_phase_range(acm_ctx* c, int z0, int z1)
             a.N = (unsigned)c->N;
             a.one_minus_omega = (T)(1.0 - 1.0 / (3.0 * c->M + 0.5));
             a.inv_xi = (T)(1.0 / c->xi);
-            cudaError_t e = launch_phase_mom<T>(c->Qh, c->walls != 0, lb_launch(c, z1 - z0, 1), a);
+            const bool march = mom_march(c);
+            if (march) a.g = geom_of(c, false, z0, z1);
+            cudaError_t e = march ? launch_phase_mom_march<T>(c->Qh, c->walls != 0, mom_zchunk(c, z1 - z0), c->stream, a)
+                                  : launch_phase_mom<T>(c->Qh, c->walls != 0, lb_launch(c, z1 - z0, 1), a);
             c->phase_planes += z1 - z0;
-            return check_launch(c, "phase_mom_kernel", e);
+            return check_launch(c, march ? "phase_mom_march_kernel" : "phase_mom_kernel", e);
         } else return fail(ACM_EINVAL, "ACM_OPT_MOMENTS is fp64 only");
     }
     PhaseArgs<T> a;
@@ -290,9 +318,12 @@ static int launch_hydro_range(acm_ctx* c, int z0, int z1)
             ma.h.g = geom_of(c, lb_linear(c, 1), z0, z1);
             ma.Ksrc = wsp<T>(c, c->offG[c->curG]); ma.Kdst = wsp<T>(c, c->offG[c->curG ^ 1]);
             ma.Uin = wsp<T>(c, c->offU[c->curU]); ma.Uout = wsp<T>(c, c->offU[c->curU ^ 1]);
-            cudaError_t e = launch_hydro_mom<T>(c->Qg, c->walls != 0, c->stG == ST_IN, lb_launch(c, z1 - z0, 1), ma);
+            const bool march = mom_march(c) && c->stG != ST_IN;      // the first step after acm_init (no streaming) stays direct
+            if (march) ma.h.g = geom_of(c, false, z0, z1);
+            cudaError_t e = march ? launch_hydro_mom_march<T>(c->Qg, c->walls != 0, mom_zchunk(c, z1 - z0), c->stream, ma)
+                                  : launch_hydro_mom<T>(c->Qg, c->walls != 0, c->stG == ST_IN, lb_launch(c, z1 - z0, 1), ma);
             c->hydro_planes += z1 - z0;
-            return check_launch(c, "hydro_mom_kernel", e);
+            return check_launch(c, march ? "hydro_mom_march_kernel" : "hydro_mom_kernel", e);
         } else return fail(ACM_EINVAL, "ACM_OPT_MOMENTS is fp64 only");
     }
     const Launch l = lb_launch(c, z1 - z0, cpt);
@@ -585,6 +616,12 @@ static int create_impl(acm_ctx** out, int nx, int ny, int nz, int stencil_phase,
     c->launches = 0;
     c->steps_done = 0;
     c->subiter = 1;
+    c->uH = 0; c->mom_mode = -1; c->mom_zchunk = 0;
+    {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); sms = 0; }
+        c->sm_count = sms;
+    }
     c->phase_planes = c->hydro_planes = 0;
     c->profiling = false;
     c->ev_used = 0;
@@ -867,6 +904,16 @@ int acm_set_subiter(acm_ctx* c, int sweeps)
         return fail(ACM_EINVAL, "acm_set_subiter: not available for slabs or with ACM_OPT_UNFUSED");
     if (c->phase_planes || c->hydro_planes) return fail(ACM_ESTATE, "acm_set_subiter: a step is partly launched (commit it first)");
     c->subiter = sweeps;
+    graphs_clear(c);
+    return ACM_OK;
+}
+
+int acm_set_moment_kernels(acm_ctx* c, int mode, int zchunk)
+{
+    ACM_CHECK_CTX(c);
+    if (!(c->options & ACM_OPT_MOMENTS)) return fail(ACM_ESTATE, "acm_set_moment_kernels: the context was not created with ACM_OPT_MOMENTS");
+    if (mode < -1 || mode > 1 || zchunk < 0) return fail(ACM_EINVAL, "acm_set_moment_kernels: mode must be -1, 0 or 1 and zchunk >= 0");
+    c->mom_mode = mode; c->mom_zchunk = zchunk;
     graphs_clear(c);
     return ACM_OK;
 }

@@ -32,6 +32,10 @@ template <typename T> cudaError_t launch_unfused_hydro(int Q, bool walls, const 
 // local: the coefficient array of g holds the cell's own incoming populations (state right after acm_init).
 template <typename T> cudaError_t launch_phase_mom(int Q, bool walls, const Launch& l, const MomPhaseArgs<T>& a);
 template <typename T> cudaError_t launch_hydro_mom(int Q, bool walls, bool local, const Launch& l, const MomHydroArgs<T>& a);
+// ... and as marching kernels: 32 x 8 tiles of columns marching along z over `zchunk` planes per block, the coefficient planes
+// staged in shared memory by cp.async (the geometry's launch range [lz0, lz1) is split into chunks; l.grid / l.block are unused)
+template <typename T> cudaError_t launch_phase_mom_march(int Q, bool walls, int zchunk, cudaStream_t stream, const MomPhaseArgs<T>& a);
+template <typename T> cudaError_t launch_hydro_mom_march(int Q, bool walls, int zchunk, cudaStream_t stream, const MomHydroArgs<T>& a);
 template <typename T> cudaError_t launch_init_mom(const Launch& l, const T* phi, const T* u, T* M, T* K, T* C, T* U0, T* U1, Geom g, size_t N);
 template <typename T> cudaError_t launch_export_h_mom(int Q, const Launch& l, const T* M, const T* C, const T* Uo, T* out, Geom g, size_t N);
 template <typename T>

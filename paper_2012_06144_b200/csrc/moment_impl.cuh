@@ -17,20 +17,66 @@
 
 namespace acm {
 
+// Where the coefficients come from.  An accessor names a cell by an index (index<DX,DY,DZ>() = the cell at that
+// offset from the calling thread's) and hands out the fields of a cell:
+//   hydrodynamic set: k(f, j), f = 0..9: A, bx, by, bz, Txx, Tyy, Tzz, Txy, Txz, Tyz
+//   phase-field set:  m(f, j), f = 0..3: A, bx, by, bz;  phi(j);  u(a, j): the velocity the collision that wrote m used
+// GlobalK / GlobalM read the arrays in global memory through L1/L2; the tile accessors of the marching kernels
+// (below) read the shared-memory window.
+template <typename T>
+struct GlobalK {
+    const T* __restrict__ K;
+    size_t N;
+    const Nbr* nb;
+    template <int DX, int DY, int DZ> __device__ __forceinline__ unsigned index() const { return nb->template at<DX, DY, DZ>(); }
+    __device__ __forceinline__ T k(int f, unsigned j) const { return __ldg(K + (size_t)f * N + j); }
+};
+
+template <typename T>
+struct GlobalM {
+    const T* __restrict__ M;
+    const T* __restrict__ C;
+    const T* __restrict__ Uo;
+    size_t N;
+    const Nbr* nb;
+    template <int DX, int DY, int DZ> __device__ __forceinline__ unsigned index() const { return nb->template at<DX, DY, DZ>(); }
+    __device__ __forceinline__ T m(int f, unsigned j) const { return __ldg(M + (size_t)f * N + j); }
+    __device__ __forceinline__ T phi(unsigned j) const { return __ldg(C + j); }
+    __device__ __forceinline__ T u(int a, unsigned j) const { return __ldg(Uo + (size_t)a * N + j); }
+};
+
+// "beyond a wall" flags of a cell (the part of Nbr the pulls need; Nbr itself qualifies too)
+struct WallFlags {
+    bool wxm, wxp, wym, wyp, wzm, wzp;
+    template <int DX, int DY, int DZ, bool WALLS>
+    __device__ __forceinline__ bool beyond() const
+    {
+        if constexpr (!WALLS) return false;
+        bool b = false;
+        if constexpr (DX < 0) b |= wxm;
+        if constexpr (DX > 0) b |= wxp;
+        if constexpr (DY < 0) b |= wym;
+        if constexpr (DY > 0) b |= wyp;
+        if constexpr (DZ < 0) b |= wzm;
+        if constexpr (DZ > 0) b |= wzp;
+        return b;
+    }
+};
+
 // index of the cell that delivers population I to the calling cell, and whether the delivery is a bounce-back
 // (then the cell itself delivers its own opposite population: same even part, odd part with the other sign)
-template <int Q, int I, bool WALLS, bool LOCAL>
-__device__ __forceinline__ unsigned mom_source(const Nbr& nb, bool& flip)
+template <int Q, int I, bool WALLS, bool LOCAL, typename Acc, typename Walls>
+__device__ __forceinline__ auto mom_source(const Acc& acc, const Walls& wf, bool& flip)
 {
     using L = Lat<Q>;
     constexpr int ex = L::ex(I), ey = L::ey(I), ez = L::ez(I);
     flip = false;
-    if constexpr (LOCAL || I == 0) return nb.at<0, 0, 0>();
+    if constexpr (LOCAL || I == 0) return acc.template index<0, 0, 0>();
     else {
         if constexpr (WALLS) {
-            if (nb.template beyond<-ex, -ey, -ez, WALLS>()) { flip = true; return nb.at<0, 0, 0>(); }
+            if (wf.template beyond<-ex, -ey, -ez, WALLS>()) { flip = true; return acc.template index<0, 0, 0>(); }
         }
-        return nb.template at<-ex, -ey, -ez>();
+        return acc.template index<-ex, -ey, -ez>();
     }
 }
 
@@ -44,59 +90,84 @@ __device__ __forceinline__ void odd_term(T& acc, bool& first, T v)
     }
 }
 
-// incoming hydrodynamic population g_I(x) / w_I rebuilt from the coefficient array K[10][N].
-// LOCAL: K holds the coefficients of the cell's own INCOMING populations (state right after acm_init, whose g is
+// incoming hydrodynamic population g_I(x) / w_I rebuilt from the coefficients.
+// LOCAL: the coefficients are those of the cell's own INCOMING populations (state right after acm_init, whose g is
 // defined pre-collision at its cell, A13/A14): no streaming.
-template <int Q, int I, typename T, bool WALLS, bool LOCAL>
-__device__ __forceinline__ T mom_pull_g(const T* __restrict__ K, size_t N, const Nbr& nb)
+template <int Q, int I, typename T, bool WALLS, bool LOCAL, typename Acc, typename Walls>
+__device__ __forceinline__ T mom_pull_g(const Acc& acc, const Walls& wf)
 {
     using L = Lat<Q>;
     constexpr int ex = L::ex(I), ey = L::ey(I), ez = L::ez(I);
     bool flip;
-    const unsigned j = mom_source<Q, I, WALLS, LOCAL>(nb, flip);
-    const T* k = K + j;
-    T E = __ldg(k);                                              // A
-    if constexpr (ex != 0) E += __ldg(k + 4 * N);                // e e : T, diagonal part
-    if constexpr (ey != 0) E += __ldg(k + 5 * N);
-    if constexpr (ez != 0) E += __ldg(k + 6 * N);
-    if constexpr (ex * ey != 0) E += T(2 * ex * ey) * __ldg(k + 7 * N);
-    if constexpr (ex * ez != 0) E += T(2 * ex * ez) * __ldg(k + 8 * N);
-    if constexpr (ey * ez != 0) E += T(2 * ey * ez) * __ldg(k + 9 * N);
+    const auto j = mom_source<Q, I, WALLS, LOCAL>(acc, wf, flip);
+    T E = acc.k(0, j);                                           // A
+    if constexpr (ex != 0) E += acc.k(4, j);                     // e e : T, diagonal part
+    if constexpr (ey != 0) E += acc.k(5, j);
+    if constexpr (ez != 0) E += acc.k(6, j);
+    if constexpr (ex * ey != 0) E += T(2 * ex * ey) * acc.k(7, j);
+    if constexpr (ex * ez != 0) E += T(2 * ex * ez) * acc.k(8, j);
+    if constexpr (ey * ez != 0) E += T(2 * ey * ez) * acc.k(9, j);
     if constexpr (I == 0) return E;
     else {
         T O = T(0);
         bool first = true;
-        if constexpr (ex != 0) odd_term<ex>(O, first, __ldg(k + 1 * N));
-        if constexpr (ey != 0) odd_term<ey>(O, first, __ldg(k + 2 * N));
-        if constexpr (ez != 0) odd_term<ez>(O, first, __ldg(k + 3 * N));
+        if constexpr (ex != 0) odd_term<ex>(O, first, acc.k(1, j));
+        if constexpr (ey != 0) odd_term<ey>(O, first, acc.k(2, j));
+        if constexpr (ez != 0) odd_term<ez>(O, first, acc.k(3, j));
         if constexpr (WALLS) return flip ? E - O : E + O;
         else return E + O;
     }
 }
 
-// incoming phase-field population h_I(x) / w_I rebuilt from M[4][N] (A, b), phi and the velocity Uo the collision
-// that wrote M used:  h*_i = w_i [A + e_i.b + 4.5 phi (e_i.u)^2],  A = phi (1 - 1.5 u^2),  b = 3 phi u + F-part + relaxed part
-template <int Q, int I, typename T, bool WALLS, bool LOCAL = false>
-__device__ __forceinline__ T mom_pull_h(const T* __restrict__ M, const T* __restrict__ C, const T* __restrict__ Uo, size_t N,
-                                        const Nbr& nb)
+// incoming phase-field population h_I(x) / w_I rebuilt from A, b, phi and the velocity the collision that wrote
+// them used:  h*_i = w_i [A + e_i.b + 4.5 phi (e_i.u)^2],  A = phi (1 - 1.5 u^2),  b = 3 phi u + forcing + relaxed part
+template <int Q, int I, typename T, bool WALLS, bool LOCAL, typename Acc, typename Walls>
+__device__ __forceinline__ T mom_pull_h(const Acc& acc, const Walls& wf)
 {
     using L = Lat<Q>;
     constexpr int ex = L::ex(I), ey = L::ey(I), ez = L::ez(I);
     bool flip;
-    const unsigned j = mom_source<Q, I, WALLS, LOCAL>(nb, flip);
-    const T* m = M + j;
-    const T A = __ldg(m);
+    const auto j = mom_source<Q, I, WALLS, LOCAL>(acc, wf, flip);
+    const T A = acc.m(0, j);
     if constexpr (I == 0) return A;
     else {
         T O = T(0), eu = T(0);
         bool fo = true, fu = true;
-        if constexpr (ex != 0) { odd_term<ex>(O, fo, __ldg(m + 1 * N)); odd_term<ex>(eu, fu, __ldg(Uo + j)); }
-        if constexpr (ey != 0) { odd_term<ey>(O, fo, __ldg(m + 2 * N)); odd_term<ey>(eu, fu, __ldg(Uo + N + j)); }
-        if constexpr (ez != 0) { odd_term<ez>(O, fo, __ldg(m + 3 * N)); odd_term<ez>(eu, fu, __ldg(Uo + 2 * N + j)); }
-        const T E = A + T(4.5) * __ldg(C + j) * (eu * eu);
+        if constexpr (ex != 0) { odd_term<ex>(O, fo, acc.m(1, j)); odd_term<ex>(eu, fu, acc.u(0, j)); }
+        if constexpr (ey != 0) { odd_term<ey>(O, fo, acc.m(2, j)); odd_term<ey>(eu, fu, acc.u(1, j)); }
+        if constexpr (ez != 0) { odd_term<ez>(O, fo, acc.m(3, j)); odd_term<ez>(eu, fu, acc.u(2, j)); }
+        const T E = A + T(4.5) * acc.phi(j) * (eu * eu);
         if constexpr (WALLS) return flip ? E - O : E + O;
         else return E + O;
     }
+}
+
+// the rest of the two cell updates, shared by the direct and the marching kernels
+// phase field: from the pulled populations h, the OLD phi at the cell and its gradient, and u: phi_new and A, b of h*
+// (the MRT branch of phase_collide, lb_math.cuh, up to the coefficients)
+template <typename T, int Q>
+__device__ __forceinline__ void phase_mom_cell(const T (&h)[Q], T c0, T gx, T gy, T gz, T ux, T uy, T uz, T one_minus_omega, T inv_xi,
+                                               T& phi, T& A, T& bx, T& by, T& bz)
+{
+    Moments<Q, T, false> m;
+    m.compute(h);
+    phi = m.m0;
+    const T g2 = gx * gx + gy * gy + gz * gz;
+    const T inv = inv_norm_or_zero(g2);
+    const T dc = c0 - T(0.5);
+    const T theta = (T(1) - T(4) * dc * dc) * inv_xi;
+    const T tnx = theta * inv * gx, tny = theta * inv * gy, tnz = theta * inv * gz;
+    const T k = T(3) * one_minus_omega;
+    const T sixth = T(1.0 / 6.0);
+    const T dxm = m.jx - phi * ux + sixth * tnx;
+    const T dym = m.jy - phi * uy + sixth * tny;
+    const T dzm = m.jz - phi * uz + sixth * tnz;
+    const T p3 = T(3) * phi;
+    const T usq = T(1.5) * (ux * ux + uy * uy + uz * uz);
+    A = phi * (T(1) - usq);
+    bx = p3 * ux + T(0.5) * tnx + k * dxm;
+    by = p3 * uy + T(0.5) * tny + k * dym;
+    bz = p3 * uz + T(0.5) * tnz + k * dzm;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -112,36 +183,19 @@ __global__ void __launch_bounds__(ACM_MAXT) phase_mom_kernel(const MomPhaseArgs<
     const unsigned idx = nb.at<0, 0, 0>();
     const size_t N = a.N;
 
+    const GlobalM<T> acc{a.Msrc, a.Csrc, a.Uold, N, &nb};
     T h[Q];
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        h[i] = T(Lat<Q>::w(i)) * mom_pull_h<Q, i, T, WALLS>(a.Msrc, a.Csrc, a.Uold, N, nb);
+        h[i] = T(Lat<Q>::w(i)) * mom_pull_h<Q, i, T, WALLS, false>(acc, nb);
     });
     const T ux = __ldg(a.U + idx), uy = __ldg(a.U + N + idx), uz = __ldg(a.U + 2 * N + idx);
     const T c0 = __ldg(a.Csrc + idx);
     T gx, gy, gz, lap_unused;
     fd_phi<Q, T, false>(a.Csrc, nb, c0, gx, gy, gz, lap_unused);
-
-    Moments<Q, T, false> m;
-    m.compute(h);
-    const T phi = m.m0;
-    // the MRT branch of phase_collide (lb_math.cuh) up to the coefficients
-    const T g2 = gx * gx + gy * gy + gz * gz;
-    const T inv = inv_norm_or_zero(g2);
-    const T dc = c0 - T(0.5);
-    const T theta = (T(1) - T(4) * dc * dc) * a.inv_xi;
-    const T tnx = theta * inv * gx, tny = theta * inv * gy, tnz = theta * inv * gz;
-    const T k = T(3) * a.one_minus_omega;
-    const T sixth = T(1.0 / 6.0);
-    const T dxm = m.jx - phi * ux + sixth * tnx;
-    const T dym = m.jy - phi * uy + sixth * tny;
-    const T dzm = m.jz - phi * uz + sixth * tnz;
-    const T p3 = T(3) * phi;
-    const T usq = T(1.5) * (ux * ux + uy * uy + uz * uz);
-    a.Mdst[idx] = phi * (T(1) - usq);
-    a.Mdst[N + idx] = p3 * ux + T(0.5) * tnx + k * dxm;
-    a.Mdst[2 * N + idx] = p3 * uy + T(0.5) * tny + k * dym;
-    a.Mdst[3 * N + idx] = p3 * uz + T(0.5) * tnz + k * dzm;
+    T phi, A, bx, by, bz;
+    phase_mom_cell<T, Q>(h, c0, gx, gy, gz, ux, uy, uz, a.one_minus_omega, a.inv_xi, phi, A, bx, by, bz);
+    a.Mdst[idx] = A; a.Mdst[N + idx] = bx; a.Mdst[2 * N + idx] = by; a.Mdst[3 * N + idx] = bz;
     a.Cdst[idx] = phi;
 }
 
@@ -158,10 +212,11 @@ __global__ void __launch_bounds__(ACM_MAXT) hydro_mom_kernel(const MomHydroArgs<
     const unsigned idx = nb.at<0, 0, 0>();
     const size_t N = a.h.N;
 
+    const GlobalK<T> acc{a.Ksrc, N, &nb};
     T g[Q];
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        g[i] = T(Lat<Q>::w(i)) * mom_pull_g<Q, i, T, WALLS, LOCAL>(a.Ksrc, N, nb);
+        g[i] = T(Lat<Q>::w(i)) * mom_pull_g<Q, i, T, WALLS, LOCAL>(acc, nb);
     });
     const T uox = __ldg(a.Uin + idx), uoy = __ldg(a.Uin + N + idx), uoz = __ldg(a.Uin + 2 * N + idx);
     const T c0 = __ldg(a.h.C + idx);
@@ -176,6 +231,211 @@ __global__ void __launch_bounds__(ACM_MAXT) hydro_mom_kernel(const MomHydroArgs<
     T* o = a.Kdst + idx;
     o[0] = k.A; o[N] = k.bx; o[2 * N] = k.by; o[3 * N] = k.bz;
     o[4 * N] = k.Txx; o[5 * N] = k.Tyy; o[6 * N] = k.Tzz; o[7 * N] = k.Txy; o[8 * N] = k.Txz; o[9 * N] = k.Tyz;
+}
+
+// ------------------------------------------------------------------------------------------
+// The marching kernels.  The direct kernels above are latency-bound: each thread issues ~110 dependent-free but
+// register-limited loads per cell through L1 (ncu: DRAM at half its rate, nothing else saturated).  Here a block owns a
+// TX x TY tile of columns and marches along z over `zchunk` planes; the coefficient planes it needs (tile + one-cell
+// halo, periodic wrap / wall clamp applied by the loader) travel global -> shared memory by cp.async into a ring of
+// four plane slots: while plane z is computed from the slots of z-1, z, z+1, plane z+2 is in flight.  One barrier per
+// plane.  Every coefficient is fetched from L2 once per tile (+ halo), the gather runs on shared memory.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void cp_async8(void* smem, const void* gmem)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+template <int TX, int TY>
+struct MomTile {
+    static constexpr int PITCH = TX + 2, ROWS = TY + 2, TILE = PITCH * ROWS, NT = TX * TY;
+    static constexpr int PER = (TILE + NT - 1) / NT;      // tile entries a thread copies per field and plane
+    static constexpr int RING = 4;
+};
+
+// coordinate of a halo / tile entry on one axis: periodic wrap or wall clamp (the mirror ghost of the phi stencil);
+// entries beyond the far end of a ragged tile are never used, they only need a valid address
+__device__ __forceinline__ int tile_coord(int v, int n, bool wall)
+{
+    if (v < 0) return wall ? 0 : n - 1;
+    if (v >= n) return (v == n && !wall) ? 0 : n - 1;
+    return v;
+}
+
+// copies of one plane: for each of NF fields (field f at base[f], plane offset zoff) the thread's entries
+template <int NF, typename TL, typename T>
+__device__ __forceinline__ void tile_load_plane(T* slot, const T* const (&base)[NF], size_t zoff, const unsigned (&src)[TL::PER], int tid)
+{
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+        const T* b = base[f] + zoff;
+#pragma unroll
+        for (int k = 0; k < TL::PER; ++k) {
+            const int e = tid + k * TL::NT;
+            if (k + 1 < TL::PER || e < TL::TILE) cp_async8(slot + f * TL::TILE + e, b + src[k]);
+        }
+    }
+}
+
+// shared-memory window as an accessor: base[d] = offset of the thread's own entry in the slot of plane z - 1 + d
+template <typename T, typename TL>
+struct TileK {
+    const T* s;
+    int base[3];
+    template <int DX, int DY, int DZ> __device__ __forceinline__ int index() const { return base[DZ + 1] + DY * TL::PITCH + DX; }
+    __device__ __forceinline__ T k(int f, int j) const { return s[j + f * TL::TILE]; }
+};
+
+template <typename T, typename TL>
+struct TileM {      // fields of a slot: 0..3 = A, b; 4 = phi; 5..7 = u
+    const T* s;
+    int base[3];
+    template <int DX, int DY, int DZ> __device__ __forceinline__ int index() const { return base[DZ + 1] + DY * TL::PITCH + DX; }
+    __device__ __forceinline__ T m(int f, int j) const { return s[j + f * TL::TILE]; }
+    __device__ __forceinline__ T phi(int j) const { return s[j + 4 * TL::TILE]; }
+    __device__ __forceinline__ T u(int a, int j) const { return s[j + (5 + a) * TL::TILE]; }
+    template <int DX, int DY, int DZ> __device__ __forceinline__ T get() const { return phi(index<DX, DY, DZ>()); }   // fd_phi_acc
+};
+
+// what the two marching kernels share: the block's tile, the thread's loader entries, the z range
+template <typename TL>
+struct MarchSetup {
+    int x, y, tid, zb, ze;
+    bool active;
+    unsigned src[TL::PER];
+    unsigned plane;      // nx * ny
+    __device__ __forceinline__ void init(const Geom& g, int zchunk)
+    {
+        tid = threadIdx.y * blockDim.x + threadIdx.x;
+        const int x0 = blockIdx.x * (TL::PITCH - 2), y0 = blockIdx.y * (TL::ROWS - 2);
+        x = x0 + threadIdx.x; y = y0 + threadIdx.y;
+        active = x < g.nx && y < g.ny;
+        zb = g.lz0 + blockIdx.z * zchunk;
+        ze = min(zb + zchunk, g.lz1);
+        plane = (unsigned)(g.nx * g.ny);
+#pragma unroll
+        for (int k = 0; k < TL::PER; ++k) {
+            const int e = min(tid + k * TL::NT, TL::TILE - 1);
+            const int r = e / TL::PITCH, c = e - r * TL::PITCH;
+            const int gx = tile_coord(x0 + c - 1, g.nx, (g.walls & ACM_WALL_X) != 0);
+            const int gy = tile_coord(y0 + r - 1, g.ny, (g.walls & ACM_WALL_Y) != 0);
+            src[k] = (unsigned)(gy * g.nx + gx);
+        }
+    }
+    // offset of plane zz (zb - 1 <= zz <= ze): periodic wrap inside [zlo, zhi) or wall clamp
+    __device__ __forceinline__ size_t zoff(const Geom& g, int zz) const
+    {
+        int z = zz;
+        if (z < g.zlo) z = (g.walls & WALL_ZLO) ? g.zlo : g.zhi - 1;
+        else if (z >= g.zhi) z = (g.walls & WALL_ZHI) ? g.zhi - 1 : g.zlo;
+        return (size_t)z * plane;
+    }
+    __device__ __forceinline__ int slot_of(int zz) const { return (zz - zb + 1) & (TL::RING - 1); }
+};
+
+template <typename T, int Q, bool WALLS, int TX, int TY>
+__global__ void __launch_bounds__(TX * TY, 2) phase_mom_march_kernel(const MomPhaseArgs<T> a, int zchunk)
+{
+    using TL = MomTile<TX, TY>;
+    constexpr int NF = 8;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* s = reinterpret_cast<T*>(smem_raw);      // [RING][NF][TILE]
+    const Geom& g = a.g;
+    const size_t N = a.N;
+    MarchSetup<TL> ms;
+    ms.init(g, zchunk);
+    if (ms.zb >= ms.ze) return;
+    const T* const base[NF] = {a.Msrc, a.Msrc + N, a.Msrc + 2 * N, a.Msrc + 3 * N, a.Csrc, a.Uold, a.Uold + N, a.Uold + 2 * N};
+    for (int zz = ms.zb - 1; zz <= ms.zb + 1; ++zz)
+        tile_load_plane<NF, TL>(s + ms.slot_of(zz) * NF * TL::TILE, base, ms.zoff(g, zz), ms.src, ms.tid);
+    cp_async_commit();
+
+    const int own = (threadIdx.y + 1) * TL::PITCH + threadIdx.x + 1;
+    WallFlags wf;
+    wf.wxm = WALLS && (g.walls & ACM_WALL_X) && ms.x == 0; wf.wxp = WALLS && (g.walls & ACM_WALL_X) && ms.x == g.nx - 1;
+    wf.wym = WALLS && (g.walls & ACM_WALL_Y) && ms.y == 0; wf.wyp = WALLS && (g.walls & ACM_WALL_Y) && ms.y == g.ny - 1;
+    const unsigned col = (unsigned)(ms.y * g.nx + ms.x);
+    for (int z = ms.zb; z < ms.ze; ++z) {
+        cp_async_wait_all();
+        __syncthreads();      // planes z-1 .. z+1 have landed for everyone, and everyone is done with the slot of z-2
+        if (z + 2 <= ms.ze) tile_load_plane<NF, TL>(s + ms.slot_of(z + 2) * NF * TL::TILE, base, ms.zoff(g, z + 2), ms.src, ms.tid);
+        cp_async_commit();
+        if (!ms.active) continue;
+        wf.wzm = WALLS && (g.walls & WALL_ZLO) && z == g.zlo; wf.wzp = WALLS && (g.walls & WALL_ZHI) && z == g.zhi - 1;
+        TileM<T, TL> acc;
+        acc.s = s;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) acc.base[d] = ms.slot_of(z - 1 + d) * NF * TL::TILE + own;
+        T h[Q];
+        static_for<0, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            h[i] = T(Lat<Q>::w(i)) * mom_pull_h<Q, i, T, WALLS, false>(acc, wf);
+        });
+        const unsigned idx = (unsigned)z * ms.plane + col;
+        const T ux = __ldg(a.U + idx), uy = __ldg(a.U + N + idx), uz = __ldg(a.U + 2 * N + idx);
+        const T c0 = acc.phi(acc.base[1]);
+        T gx, gy, gz, lap_unused;
+        fd_phi_acc<Q, T, false>(acc, c0, gx, gy, gz, lap_unused);
+        T phi, A, bx, by, bz;
+        phase_mom_cell<T, Q>(h, c0, gx, gy, gz, ux, uy, uz, a.one_minus_omega, a.inv_xi, phi, A, bx, by, bz);
+        a.Mdst[idx] = A; a.Mdst[N + idx] = bx; a.Mdst[2 * N + idx] = by; a.Mdst[3 * N + idx] = bz;
+        a.Cdst[idx] = phi;
+    }
+}
+
+template <typename T, int Q, bool WALLS, int HVAR, int TX, int TY>
+__global__ void __launch_bounds__(TX * TY, 2) hydro_mom_march_kernel(const MomHydroArgs<T> a, int zchunk)
+{
+    using TL = MomTile<TX, TY>;
+    constexpr int NF = 10;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* s = reinterpret_cast<T*>(smem_raw);      // [RING][NF][TILE]
+    const Geom& g = a.h.g;
+    const size_t N = a.h.N;
+    MarchSetup<TL> ms;
+    ms.init(g, zchunk);
+    if (ms.zb >= ms.ze) return;
+    const T* const base[NF] = {a.Ksrc, a.Ksrc + N, a.Ksrc + 2 * N, a.Ksrc + 3 * N, a.Ksrc + 4 * N,
+                               a.Ksrc + 5 * N, a.Ksrc + 6 * N, a.Ksrc + 7 * N, a.Ksrc + 8 * N, a.Ksrc + 9 * N};
+    for (int zz = ms.zb - 1; zz <= ms.zb + 1; ++zz)
+        tile_load_plane<NF, TL>(s + ms.slot_of(zz) * NF * TL::TILE, base, ms.zoff(g, zz), ms.src, ms.tid);
+    cp_async_commit();
+
+    const int own = (threadIdx.y + 1) * TL::PITCH + threadIdx.x + 1;
+    for (int z = ms.zb; z < ms.ze; ++z) {
+        cp_async_wait_all();
+        __syncthreads();
+        if (z + 2 <= ms.ze) tile_load_plane<NF, TL>(s + ms.slot_of(z + 2) * NF * TL::TILE, base, ms.zoff(g, z + 2), ms.src, ms.tid);
+        cp_async_commit();
+        if (!ms.active) continue;
+        Nbr nb;      // the phi stencil (one field) still goes through L1/L2, like in the population kernels
+        nb.setup<WALLS>(g, ms.x, ms.y, z);
+        TileK<T, TL> acc;
+        acc.s = s;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) acc.base[d] = ms.slot_of(z - 1 + d) * NF * TL::TILE + own;
+        T gp[Q];
+        static_for<0, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            gp[i] = T(Lat<Q>::w(i)) * mom_pull_g<Q, i, T, WALLS, false>(acc, nb);
+        });
+        const unsigned idx = nb.at<0, 0, 0>();
+        const T uox = __ldg(a.Uin + idx), uoy = __ldg(a.Uin + N + idx), uoz = __ldg(a.Uin + 2 * N + idx);
+        const T c0 = __ldg(a.h.C + idx);
+        T gpx, gpy, gpz, lap;
+        fd_phi<Q, T, true>(a.h.C, nb, c0, gpx, gpy, gpz, lap);
+        Moments<Q, T, true> m;
+        m.compute(gp);
+        const HydroCell<T> hc = hydro_velocity<T, Q, HVAR>(m, c0, gpx, gpy, gpz, lap, uox, uoy, uoz, a.h);
+        a.Uout[idx] = hc.ux; a.Uout[N + idx] = hc.uy; a.Uout[2 * N + idx] = hc.uz;
+        const Coeffs<T> k = hydro_coeffs<T, Q, HVAR>(m, hc, a.h);
+        T* o = a.Kdst + idx;
+        o[0] = k.A; o[N] = k.bx; o[2 * N] = k.by; o[3 * N] = k.bz;
+        o[4 * N] = k.Txx; o[5 * N] = k.Tyy; o[6 * N] = k.Tzz; o[7 * N] = k.Txy; o[8 * N] = k.Txz; o[9 * N] = k.Tyz;
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -214,9 +474,10 @@ __global__ void export_h_mom_kernel(const T* __restrict__ M, const T* __restrict
     Nbr nb;
     nb.setup<true>(g, x, y, z);
     const unsigned idx = nb.at<0, 0, 0>();
+    const GlobalM<T> acc{M, C, Uo, N, &nb};
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        out[(size_t)i * N + idx] = T(Lat<Q>::w(i)) * mom_pull_h<Q, i, T, false, true>(M, C, Uo, N, nb);
+        out[(size_t)i * N + idx] = T(Lat<Q>::w(i)) * mom_pull_h<Q, i, T, false, true>(acc, nb);
     });
 }
 
@@ -228,10 +489,11 @@ __global__ void export_g_mom_kernel(const T* __restrict__ K, const T* __restrict
     Nbr nb;
     nb.setup<true>(g, x, y, z);
     const unsigned idx = nb.at<0, 0, 0>();
+    const GlobalK<T> acc{K, N, &nb};
     T f[Q];
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        f[i] = T(Lat<Q>::w(i)) * mom_pull_g<Q, i, T, true, LOCAL>(K, N, nb);
+        f[i] = T(Lat<Q>::w(i)) * mom_pull_g<Q, i, T, true, LOCAL>(acc, nb);
     });
     if (out) static_for<0, Q>([&](auto ic) { constexpr int i = decltype(ic)::value; out[(size_t)i * N + idx] = f[i]; });
     if (p) {
@@ -309,6 +571,60 @@ cudaError_t launch_export_g_mom(int Q, bool local, const Launch& l, const T* K, 
     return cudaGetLastError();
 }
 
+// marching kernels: 32 x 8 tiles of columns, `zchunk` planes per block
+constexpr int MARCH_TX = 32, MARCH_TY = 8;
+
+template <typename K>
+static cudaError_t march_smem(K kernel, size_t bytes)
+{
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+static Launch march_launch(const Geom& g, int zchunk, cudaStream_t stream)
+{
+    const int planes = g.lz1 - g.lz0;
+    return Launch{dim3((g.nx + MARCH_TX - 1) / MARCH_TX, (g.ny + MARCH_TY - 1) / MARCH_TY, (planes + zchunk - 1) / zchunk), dim3(MARCH_TX, MARCH_TY, 1), stream};
+}
+
+template <typename T>
+cudaError_t launch_phase_mom_march(int Q, bool walls, int zchunk, cudaStream_t stream, const MomPhaseArgs<T>& a)
+{
+    using TL = MomTile<MARCH_TX, MARCH_TY>;
+    const size_t bytes = (size_t)TL::RING * 8 * TL::TILE * sizeof(T);
+    const Launch l = march_launch(a.g, zchunk, stream);
+    cudaError_t e = cudaSuccess;
+    ACM_MOM_DISPATCH_Q(Q, QQ, {
+        if (walls) { auto k = phase_mom_march_kernel<T, QQ, true, MARCH_TX, MARCH_TY>; e = march_smem(k, bytes); if (e == cudaSuccess) k<<<l.grid, l.block, bytes, l.stream>>>(a, zchunk); }
+        else { auto k = phase_mom_march_kernel<T, QQ, false, MARCH_TX, MARCH_TY>; e = march_smem(k, bytes); if (e == cudaSuccess) k<<<l.grid, l.block, bytes, l.stream>>>(a, zchunk); }
+    });
+    return e != cudaSuccess ? e : cudaGetLastError();
+}
+
+template <typename T, int Q, bool WALLS>
+static cudaError_t launch_hydro_mom_march_q(int zchunk, cudaStream_t stream, const MomHydroArgs<T>& a)
+{
+    using TL = MomTile<MARCH_TX, MARCH_TY>;
+    const size_t bytes = (size_t)TL::RING * 10 * TL::TILE * sizeof(T);
+    const Launch l = march_launch(a.h.g, zchunk, stream);
+    cudaError_t e;
+    if (a.h.bulk_one || a.h.subiter > 1) { auto k = hydro_mom_march_kernel<T, Q, WALLS, 1, MARCH_TX, MARCH_TY>; e = march_smem(k, bytes); if (e == cudaSuccess) k<<<l.grid, l.block, bytes, l.stream>>>(a, zchunk); }
+    else { auto k = hydro_mom_march_kernel<T, Q, WALLS, 0, MARCH_TX, MARCH_TY>; e = march_smem(k, bytes); if (e == cudaSuccess) k<<<l.grid, l.block, bytes, l.stream>>>(a, zchunk); }
+    return e != cudaSuccess ? e : cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_hydro_mom_march(int Q, bool walls, int zchunk, cudaStream_t stream, const MomHydroArgs<T>& a)
+{
+    cudaError_t e = cudaSuccess;
+    ACM_MOM_DISPATCH_Q(Q, QQ, {
+        if (walls) e = launch_hydro_mom_march_q<T, QQ, true>(zchunk, stream, a);
+        else e = launch_hydro_mom_march_q<T, QQ, false>(zchunk, stream, a);
+    });
+    return e;
+}
+
+template cudaError_t launch_phase_mom_march<ACM_T>(int, bool, int, cudaStream_t, const MomPhaseArgs<ACM_T>&);
+template cudaError_t launch_hydro_mom_march<ACM_T>(int, bool, int, cudaStream_t, const MomHydroArgs<ACM_T>&);
 template cudaError_t launch_phase_mom<ACM_T>(int, bool, const Launch&, const MomPhaseArgs<ACM_T>&);
 template cudaError_t launch_hydro_mom<ACM_T>(int, bool, bool, const Launch&, const MomHydroArgs<ACM_T>&);
 template cudaError_t launch_init_mom<ACM_T>(const Launch&, const ACM_T*, const ACM_T*, ACM_T*, ACM_T*, ACM_T*, ACM_T*, ACM_T*, Geom, size_t);

@@ -71,11 +71,21 @@ def test_workspace_bytes_and_argument_checks():
         return lib.acm_create_opt(ctypes.byref(h2), 8, 8, 8, 15, 19, 1.0, 1e-3, 1e-4, 5.0, 0.02, 1 / 60, 1 / 60, g, 0, 0, options,
                                   fake_ws, None)
     assert create_opt(binding.ACM_OPT_BULK_ONE | binding.ACM_OPT_UNFUSED) == binding.ACM_EINVAL
-    assert create_opt(16) == binding.ACM_EINVAL
+    assert create_opt(32) == binding.ACM_EINVAL                       # unknown option bit
+    # moment representation: fp64 two-grid fused kernels with the MRT phase-field collision only
+    for other in (binding.ACM_OPT_INPLACE, binding.ACM_OPT_UNFUSED, binding.ACM_OPT_PHASE_SRT):
+        assert create_opt(binding.ACM_OPT_MOMENTS | other) == binding.ACM_EINVAL
+    assert lib.acm_workspace_bytes_opt(8, 8, 8, 15, 19, 1, binding.ACM_OPT_MOMENTS) == 0
+    assert create_opt(binding.ACM_OPT_MOMENTS | binding.ACM_OPT_BULK_ONE) == binding.ACM_OK
+    assert lib.acm_set_moment_kernels(h2, 2, 0) == binding.ACM_EINVAL and lib.acm_set_moment_kernels(h2, 1, -1) == binding.ACM_EINVAL
+    assert lib.acm_set_moment_kernels(h2, 1, 16) == binding.ACM_OK and lib.acm_set_moment_kernels(h2, -1, 0) == binding.ACM_OK
+    assert lib.acm_set_cells_per_thread(h2, 2, 2) == binding.ACM_EINVAL
+    lib.acm_destroy(h2)
     assert create_opt(binding.ACM_OPT_BULK_ONE | binding.ACM_OPT_INPLACE | binding.ACM_OPT_PHASE_SRT) == binding.ACM_OK
     lib.acm_destroy(h2)
     assert create_opt(binding.ACM_OPT_UNFUSED) == binding.ACM_OK
     assert lib.acm_set_subiter(h2, 2) == binding.ACM_EINVAL           # Algorithm 1 evaluates the forces in two kernels
+    assert lib.acm_set_moment_kernels(h2, 1, 0) == binding.ACM_ESTATE  # not a moment-representation context
     lib.acm_destroy(h2)
 
 

@@ -58,8 +58,11 @@ SHAPES = [
 ]
 
 
+@pytest.mark.parametrize("march", [0, 1, 3], ids=["direct", "march", "march-zchunk3"])
 @pytest.mark.parametrize("nx,ny,nz,Qh,Qg,walls,grav,block", SHAPES)
-def test_first_steps_pdf_parity(nx, ny, nz, Qh, Qg, walls, grav, block):
+def test_first_steps_pdf_parity(nx, ny, nz, Qh, Qg, walls, grav, block, march):
+    """march: the marching kernels (shared-memory window) forced on these small ragged grids -- one tile wider than the
+    grid, several tiles with a ragged last one, z ranges of one chunk and of chunks of 3 planes with a ragged last one."""
     p = Params(nx=nx, ny=ny, nz=nz, stencil_phase=Qh, stencil_hydro=Qg, wall_flags=walls, gravity=grav,
                rho_H=1.0, rho_L=1e-3, sigma=1e-4, nu_H=0.05, nu_L=1 / 60)
     phi, u, _, _ = random_state(p, seed=11)
@@ -67,6 +70,7 @@ def test_first_steps_pdf_parity(nx, ny, nz, Qh, Qg, walls, grav, block):
     o.init(phi, u)
     a = _acm(p)
     a.set_block(*block)
+    a.set_moment_kernels(1 if march else 0, march if march > 1 else 0)
     a.init(_dev(phi), _dev(u))
     dh, dg = _pdf_diff(o, a)
     assert dh <= 1e-15 and dg <= 1e-15, (dh, dg)
@@ -80,8 +84,9 @@ def test_first_steps_pdf_parity(nx, ny, nz, Qh, Qg, walls, grav, block):
         assert max(_fields_diff(o, a)) <= k * TOL_PDF_1STEP
 
 
+@pytest.mark.parametrize("march", [0, 1], ids=["direct", "march"])
 @pytest.mark.parametrize("case", ["config1", "walls", "config3", "config5", "mu100"])
-def test_100_steps(case):
+def test_100_steps(case, march):
     """phi, u, p within 1e-10 of the oracle after 99 and 100 steps; sum(phi) conserved."""
     if case == "config1":
         p, phi, u = inputs.config1()
@@ -98,6 +103,7 @@ def test_100_steps(case):
     o = Oracle.from_params(p)
     o.init(phi, u)
     a = _acm(p)
+    a.set_moment_kernels(march, 0)
     a.init(_dev(phi), _dev(u))
     o.step(99)
     a.step(99)
@@ -111,12 +117,14 @@ def test_100_steps(case):
     assert abs(a.phi_mass() - o.phi_mass()) / m0 < 1e-13
 
 
-def test_d2q9_100_steps():
+@pytest.mark.parametrize("march", [0, 1], ids=["direct", "march"])
+def test_d2q9_100_steps(march):
     p = Params(nx=48, ny=40, nz=1, stencil_phase=9, stencil_hydro=9, wall_flags=inputs.WALL_Y, gravity=(1e-6, 0.0, 0.0))
     phi = inputs.sphere_phi(p, (24.0, 17.0, 0.5), 9.0, heavy_inside=True)
     o = Oracle.from_params(p)
     o.init(phi, inputs.zeros_u(p))
     a = _acm(p)
+    a.set_moment_kernels(march, 0)
     a.init(_dev(phi), _dev(inputs.zeros_u(p)))
     for n in (1, 1, 98):
         o.step(n)
@@ -133,6 +141,7 @@ def test_operator_variants(variant):
     o = Oracle.from_params(p, **kw)
     o.init(phi, u)
     a = _acm(p, **kw)
+    a.set_moment_kernels(1, 7)
     a.init(_dev(phi), _dev(u))
     o.step(1)
     a.step(1)
@@ -175,16 +184,23 @@ def test_graph_replay_is_bit_identical():
 
 
 def test_same_trajectory_as_the_population_kernels():
-    """Both storage forms follow the same time step: after 100 steps they differ by rounding only."""
-    p, phi, u = inputs.scaled_config3(32)
+    """Both storage forms follow the same time step: after 100 steps they differ by rounding only; the direct and the
+    marching kernels evaluate the same expressions in the same order: bit-identical (walls on one axis, ragged tiles)."""
+    p, phi, u = inputs.scaled_config3(36)
+    p = dataclasses.replace(p, wall_flags=inputs.WALL_Z, gravity=(0.0, 0.0, -1e-6))
     out = []
-    for moments in (False, True):
+    for moments, march in ((False, 0), (True, 0), (True, 1), (True, 5)):
         a = _acm(p, moments=moments)
+        if moments:
+            a.set_moment_kernels(1 if march else 0, march if march > 1 else 0)
         a.init(_dev(phi), _dev(u))
         a.step(100)
-        out.append([t.cpu().numpy() for t in a.fields()])
-    for x, y in zip(*out):
+        out.append([t.cpu().numpy() for t in a.fields()] + [t.cpu().numpy() for t in a.get_pdfs()])
+    for x, y in zip(out[0], out[1]):
         assert np.abs(x - y).max() <= 1e-12
+    for other in out[2:]:
+        for x, y in zip(out[1], other):
+            assert (x == y).all()
 
 
 def test_workspace_and_errors():
