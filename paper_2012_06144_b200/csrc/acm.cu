@@ -178,6 +178,7 @@ static Launch lb_launch(const acm_ctx* c, int nplanes, int cpt) { return launch_
 // the two extra planes a chunk reads.
 static bool mom_march(const acm_ctx* c)
 {
+    if (c->nx % 2 != 0) return false;      // their loader copies aligned pairs of cells
     if (c->mom_mode >= 0) return c->mom_mode == 1;
     return c->Qh != 9 && (size_t)c->nx * c->ny * c->nzl >= ((size_t)1 << 21);
 }

@@ -12,6 +12,8 @@
 // traffic: 8 (11 + 5) = 128 B (phase) + 8 (14 + 13) = 216 B (hydro) per cell and step for every lattice, instead of
 // 280 + 360 B (D3Q15 + D3Q19) or 472 + 488 B (D3Q27 + D3Q27).  The price is the gather: a pulled population needs up
 // to 6 (g) / 8 (h) values of the neighbour instead of one, served by L1/L2.
+#include <cstdlib>
+
 #include "kernels.h"
 #include "lb_math.cuh"
 
@@ -246,14 +248,23 @@ __device__ __forceinline__ void cp_async8(void* smem, const void* gmem)
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem) : "memory");
 }
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem)      // bypasses L1: nothing of the stream is held there
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-template <int TX, int TY>
+// Tile of one field in a plane slot: ROWS rows (tile + one halo row on each side) of PITCH elements; the cell with
+// local x sits in column x + 2, so that the interior starts 16-byte aligned: [pad, halo, TX interior, halo, pad].
+// A row is copied by LPR lanes: TX/2 aligned 16-byte chunks and the two halo elements.
+template <int TX, int TY, int RING_ = 4>
 struct MomTile {
-    static constexpr int PITCH = TX + 2, ROWS = TY + 2, TILE = PITCH * ROWS, NT = TX * TY;
-    static constexpr int PER = (TILE + NT - 1) / NT;      // tile entries a thread copies per field and plane
-    static constexpr int RING = 4;
+    static constexpr int PITCH = TX + 4, ROWS = TY + 2, TILE = PITCH * ROWS, NT = TX * TY;
+    static constexpr int LPR = TX / 2 + 2, LANES = LPR * ROWS;
+    static constexpr int RING = RING_;                    // plane slots: 4 = the next plane loads under the computation, 3 = after it
+    static_assert(TX % 2 == 0 && LANES <= NT, "one copy lane per thread");
 };
 
 // coordinate of a halo / tile entry on one axis: periodic wrap or wall clamp (the mirror ghost of the phi stencil);
@@ -265,28 +276,74 @@ __device__ __forceinline__ int tile_coord(int v, int n, bool wall)
     return v;
 }
 
-// copies of one plane: for each of NF fields (field f at base[f], plane offset zoff) the thread's entries
-template <int NF, typename TL, typename T>
-__device__ __forceinline__ void tile_load_plane(T* slot, const T* const (&base)[NF], size_t zoff, const unsigned (&src)[TL::PER], int tid)
-{
-#pragma unroll
-    for (int f = 0; f < NF; ++f) {
-        const T* b = base[f] + zoff;
-#pragma unroll
-        for (int k = 0; k < TL::PER; ++k) {
-            const int e = tid + k * TL::NT;
-            if (k + 1 < TL::PER || e < TL::TILE) cp_async8(slot + f * TL::TILE + e, b + src[k]);
+// what the two marching kernels share: the block's tile, the thread's copy lane, the z range (needs nx even)
+template <typename TL>
+struct MarchSetup {
+    int x, y, zb, ze;
+    bool active;         // the thread's column lies inside the grid
+    int copy;            // 0: no copy lane, 8 / 16: bytes of the thread's copy per field and plane
+    unsigned src, dst;   // its source offset inside a plane, its destination inside a field tile
+    unsigned plane;      // nx * ny
+    __device__ __forceinline__ void init(const Geom& g, int zchunk)
+    {
+        const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+        const int x0 = blockIdx.x * (TL::PITCH - 4), y0 = blockIdx.y * (TL::ROWS - 2);
+        x = x0 + threadIdx.x; y = y0 + threadIdx.y;
+        active = x < g.nx && y < g.ny;
+        zb = g.lz0 + blockIdx.z * zchunk;
+        ze = min(zb + zchunk, g.lz1);
+        plane = (unsigned)(g.nx * g.ny);
+        copy = 0; src = dst = 0;
+        if (tid < TL::LANES) {
+            const int r = tid / TL::LPR, l = tid - r * TL::LPR;
+            const int gy = tile_coord(y0 + r - 1, g.ny, (g.walls & ACM_WALL_Y) != 0);
+            const bool wx = (g.walls & ACM_WALL_X) != 0;
+            int gx, col;
+            if (l < TL::LPR - 2) {            // chunk of two interior cells; beyond the end of a ragged row only its first element
+                gx = x0 + 2 * l; col = 2 * l + 2;      // (the x + 1 neighbour of the last cell) is ever used
+                copy = gx + 1 < g.nx ? 16 : 8;
+                if (copy == 8) gx = tile_coord(gx, g.nx, wx);
+            } else if (l == TL::LPR - 2) { gx = tile_coord(x0 - 1, g.nx, wx); col = 1; copy = 8; }
+            else { gx = tile_coord(x0 + TL::PITCH - 4, g.nx, wx); col = TL::PITCH - 2; copy = 8; }
+            src = (unsigned)(gy * g.nx + gx);
+            dst = (unsigned)(r * TL::PITCH + col);
         }
     }
-}
+    // offset of plane zz (zb - 1 <= zz <= ze): periodic wrap inside [zlo, zhi) or wall clamp
+    __device__ __forceinline__ size_t zoff(const Geom& g, int zz) const
+    {
+        int z = zz;
+        if (z < g.zlo) z = (g.walls & WALL_ZLO) ? g.zlo : g.zhi - 1;
+        else if (z >= g.zhi) z = (g.walls & WALL_ZHI) ? g.zhi - 1 : g.zlo;
+        return (size_t)z * plane;
+    }
+    __device__ __forceinline__ int slot_of(int zz) const { return TL::RING == 4 ? ((zz - zb + 1) & 3) : (zz - zb + 1) % TL::RING; }
+    // copies of one plane: for each of NF fields (field f at base[f]) the thread's lane
+    template <int NF, typename T>
+    __device__ __forceinline__ void load_plane(T* slot, const T* const (&base)[NF], const Geom& g, int zz) const
+    {
+        if (copy == 0) return;
+        const size_t off = zoff(g, zz) + src;
+        T* d = slot + dst;
+        if (copy == 16) {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) cp_async16(d + f * TL::TILE, base[f] + off);
+        } else {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) cp_async8(d + f * TL::TILE, base[f] + off);
+        }
+    }
+};
 
 // shared-memory window as an accessor: base[d] = offset of the thread's own entry in the slot of plane z - 1 + d
 template <typename T, typename TL>
-struct TileK {
+struct TileK {      // fields of a slot: 0..9 = A, b, T; 10 = phi
     const T* s;
     int base[3];
     template <int DX, int DY, int DZ> __device__ __forceinline__ int index() const { return base[DZ + 1] + DY * TL::PITCH + DX; }
     __device__ __forceinline__ T k(int f, int j) const { return s[j + f * TL::TILE]; }
+    __device__ __forceinline__ T phi(int j) const { return s[j + 10 * TL::TILE]; }
+    template <int DX, int DY, int DZ> __device__ __forceinline__ T get() const { return phi(index<DX, DY, DZ>()); }   // fd_phi_acc
 };
 
 template <typename T, typename TL>
@@ -298,42 +355,6 @@ struct TileM {      // fields of a slot: 0..3 = A, b; 4 = phi; 5..7 = u
     __device__ __forceinline__ T phi(int j) const { return s[j + 4 * TL::TILE]; }
     __device__ __forceinline__ T u(int a, int j) const { return s[j + (5 + a) * TL::TILE]; }
     template <int DX, int DY, int DZ> __device__ __forceinline__ T get() const { return phi(index<DX, DY, DZ>()); }   // fd_phi_acc
-};
-
-// what the two marching kernels share: the block's tile, the thread's loader entries, the z range
-template <typename TL>
-struct MarchSetup {
-    int x, y, tid, zb, ze;
-    bool active;
-    unsigned src[TL::PER];
-    unsigned plane;      // nx * ny
-    __device__ __forceinline__ void init(const Geom& g, int zchunk)
-    {
-        tid = threadIdx.y * blockDim.x + threadIdx.x;
-        const int x0 = blockIdx.x * (TL::PITCH - 2), y0 = blockIdx.y * (TL::ROWS - 2);
-        x = x0 + threadIdx.x; y = y0 + threadIdx.y;
-        active = x < g.nx && y < g.ny;
-        zb = g.lz0 + blockIdx.z * zchunk;
-        ze = min(zb + zchunk, g.lz1);
-        plane = (unsigned)(g.nx * g.ny);
-#pragma unroll
-        for (int k = 0; k < TL::PER; ++k) {
-            const int e = min(tid + k * TL::NT, TL::TILE - 1);
-            const int r = e / TL::PITCH, c = e - r * TL::PITCH;
-            const int gx = tile_coord(x0 + c - 1, g.nx, (g.walls & ACM_WALL_X) != 0);
-            const int gy = tile_coord(y0 + r - 1, g.ny, (g.walls & ACM_WALL_Y) != 0);
-            src[k] = (unsigned)(gy * g.nx + gx);
-        }
-    }
-    // offset of plane zz (zb - 1 <= zz <= ze): periodic wrap inside [zlo, zhi) or wall clamp
-    __device__ __forceinline__ size_t zoff(const Geom& g, int zz) const
-    {
-        int z = zz;
-        if (z < g.zlo) z = (g.walls & WALL_ZLO) ? g.zlo : g.zhi - 1;
-        else if (z >= g.zhi) z = (g.walls & WALL_ZHI) ? g.zhi - 1 : g.zlo;
-        return (size_t)z * plane;
-    }
-    __device__ __forceinline__ int slot_of(int zz) const { return (zz - zb + 1) & (TL::RING - 1); }
 };
 
 template <typename T, int Q, bool WALLS, int TX, int TY>
@@ -350,10 +371,10 @@ __global__ void __launch_bounds__(TX * TY, 2) phase_mom_march_kernel(const MomPh
     if (ms.zb >= ms.ze) return;
     const T* const base[NF] = {a.Msrc, a.Msrc + N, a.Msrc + 2 * N, a.Msrc + 3 * N, a.Csrc, a.Uold, a.Uold + N, a.Uold + 2 * N};
     for (int zz = ms.zb - 1; zz <= ms.zb + 1; ++zz)
-        tile_load_plane<NF, TL>(s + ms.slot_of(zz) * NF * TL::TILE, base, ms.zoff(g, zz), ms.src, ms.tid);
+        ms.load_plane(s + ms.slot_of(zz) * NF * TL::TILE, base, g, zz);
     cp_async_commit();
 
-    const int own = (threadIdx.y + 1) * TL::PITCH + threadIdx.x + 1;
+    const int own = (threadIdx.y + 1) * TL::PITCH + threadIdx.x + 2;
     WallFlags wf;
     wf.wxm = WALLS && (g.walls & ACM_WALL_X) && ms.x == 0; wf.wxp = WALLS && (g.walls & ACM_WALL_X) && ms.x == g.nx - 1;
     wf.wym = WALLS && (g.walls & ACM_WALL_Y) && ms.y == 0; wf.wyp = WALLS && (g.walls & ACM_WALL_Y) && ms.y == g.ny - 1;
@@ -361,7 +382,7 @@ __global__ void __launch_bounds__(TX * TY, 2) phase_mom_march_kernel(const MomPh
     for (int z = ms.zb; z < ms.ze; ++z) {
         cp_async_wait_all();
         __syncthreads();      // planes z-1 .. z+1 have landed for everyone, and everyone is done with the slot of z-2
-        if (z + 2 <= ms.ze) tile_load_plane<NF, TL>(s + ms.slot_of(z + 2) * NF * TL::TILE, base, ms.zoff(g, z + 2), ms.src, ms.tid);
+        if (z + 2 <= ms.ze) ms.load_plane(s + ms.slot_of(z + 2) * NF * TL::TILE, base, g, z + 2);
         cp_async_commit();
         if (!ms.active) continue;
         wf.wzm = WALLS && (g.walls & WALL_ZLO) && z == g.zlo; wf.wzp = WALLS && (g.walls & WALL_ZHI) && z == g.zhi - 1;
@@ -386,11 +407,11 @@ __global__ void __launch_bounds__(TX * TY, 2) phase_mom_march_kernel(const MomPh
     }
 }
 
-template <typename T, int Q, bool WALLS, int HVAR, int TX, int TY>
-__global__ void __launch_bounds__(TX * TY, 2) hydro_mom_march_kernel(const MomHydroArgs<T> a, int zchunk)
+template <typename T, int Q, bool WALLS, int HVAR, int TX, int TY, int RING, int MINB>
+__global__ void __launch_bounds__(TX * TY, MINB) hydro_mom_march_kernel(const MomHydroArgs<T> a, int zchunk)
 {
-    using TL = MomTile<TX, TY>;
-    constexpr int NF = 10;
+    using TL = MomTile<TX, TY, RING>;
+    constexpr int NF = 11;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* s = reinterpret_cast<T*>(smem_raw);      // [RING][NF][TILE]
     const Geom& g = a.h.g;
@@ -399,42 +420,54 @@ __global__ void __launch_bounds__(TX * TY, 2) hydro_mom_march_kernel(const MomHy
     ms.init(g, zchunk);
     if (ms.zb >= ms.ze) return;
     const T* const base[NF] = {a.Ksrc, a.Ksrc + N, a.Ksrc + 2 * N, a.Ksrc + 3 * N, a.Ksrc + 4 * N,
-                               a.Ksrc + 5 * N, a.Ksrc + 6 * N, a.Ksrc + 7 * N, a.Ksrc + 8 * N, a.Ksrc + 9 * N};
+                               a.Ksrc + 5 * N, a.Ksrc + 6 * N, a.Ksrc + 7 * N, a.Ksrc + 8 * N, a.Ksrc + 9 * N, a.h.C};
     for (int zz = ms.zb - 1; zz <= ms.zb + 1; ++zz)
-        tile_load_plane<NF, TL>(s + ms.slot_of(zz) * NF * TL::TILE, base, ms.zoff(g, zz), ms.src, ms.tid);
+        ms.load_plane(s + ms.slot_of(zz) * NF * TL::TILE, base, g, zz);
     cp_async_commit();
 
-    const int own = (threadIdx.y + 1) * TL::PITCH + threadIdx.x + 1;
+    const int own = (threadIdx.y + 1) * TL::PITCH + threadIdx.x + 2;
+    WallFlags wf;
+    wf.wxm = WALLS && (g.walls & ACM_WALL_X) && ms.x == 0; wf.wxp = WALLS && (g.walls & ACM_WALL_X) && ms.x == g.nx - 1;
+    wf.wym = WALLS && (g.walls & ACM_WALL_Y) && ms.y == 0; wf.wyp = WALLS && (g.walls & ACM_WALL_Y) && ms.y == g.ny - 1;
+    const unsigned col = ms.active ? (unsigned)(ms.y * g.nx + ms.x) : 0u;
     for (int z = ms.zb; z < ms.ze; ++z) {
-        cp_async_wait_all();
-        __syncthreads();
-        if (z + 2 <= ms.ze) tile_load_plane<NF, TL>(s + ms.slot_of(z + 2) * NF * TL::TILE, base, ms.zoff(g, z + 2), ms.src, ms.tid);
-        cp_async_commit();
-        if (!ms.active) continue;
-        Nbr nb;      // the phi stencil (one field) still goes through L1/L2, like in the population kernels
-        nb.setup<WALLS>(g, ms.x, ms.y, z);
-        TileK<T, TL> acc;
-        acc.s = s;
-#pragma unroll
-        for (int d = 0; d < 3; ++d) acc.base[d] = ms.slot_of(z - 1 + d) * NF * TL::TILE + own;
-        T gp[Q];
-        static_for<0, Q>([&](auto ic) {
-            constexpr int i = decltype(ic)::value;
-            gp[i] = T(Lat<Q>::w(i)) * mom_pull_g<Q, i, T, WALLS, false>(acc, nb);
-        });
-        const unsigned idx = nb.at<0, 0, 0>();
+        // the velocity of the previous step (read at the cell only) is requested before the wait for the window
+        const unsigned idx = (unsigned)z * ms.plane + col;
         const T uox = __ldg(a.Uin + idx), uoy = __ldg(a.Uin + N + idx), uoz = __ldg(a.Uin + 2 * N + idx);
-        const T c0 = __ldg(a.h.C + idx);
-        T gpx, gpy, gpz, lap;
-        fd_phi<Q, T, true>(a.h.C, nb, c0, gpx, gpy, gpz, lap);
-        Moments<Q, T, true> m;
-        m.compute(gp);
-        const HydroCell<T> hc = hydro_velocity<T, Q, HVAR>(m, c0, gpx, gpy, gpz, lap, uox, uoy, uoz, a.h);
-        a.Uout[idx] = hc.ux; a.Uout[N + idx] = hc.uy; a.Uout[2 * N + idx] = hc.uz;
-        const Coeffs<T> k = hydro_coeffs<T, Q, HVAR>(m, hc, a.h);
-        T* o = a.Kdst + idx;
-        o[0] = k.A; o[N] = k.bx; o[2 * N] = k.by; o[3 * N] = k.bz;
-        o[4 * N] = k.Txx; o[5 * N] = k.Tyy; o[6 * N] = k.Tzz; o[7 * N] = k.Txy; o[8 * N] = k.Txz; o[9 * N] = k.Tyz;
+        cp_async_wait_all();
+        __syncthreads();      // planes z-1 .. z+1 have landed for everyone (RING 4: and everyone is done with the slot of z-2)
+        if constexpr (RING == 4) {
+            if (z + 2 <= ms.ze) ms.load_plane(s + ms.slot_of(z + 2) * NF * TL::TILE, base, g, z + 2);
+            cp_async_commit();
+        }
+        if (ms.active) {
+            wf.wzm = WALLS && (g.walls & WALL_ZLO) && z == g.zlo; wf.wzp = WALLS && (g.walls & WALL_ZHI) && z == g.zhi - 1;
+            TileK<T, TL> acc;
+            acc.s = s;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) acc.base[d] = ms.slot_of(z - 1 + d) * NF * TL::TILE + own;
+            T gp[Q];
+            static_for<0, Q>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                gp[i] = T(Lat<Q>::w(i)) * mom_pull_g<Q, i, T, WALLS, false>(acc, wf);
+            });
+            const T c0 = acc.phi(acc.base[1]);
+            T gpx, gpy, gpz, lap;
+            fd_phi_acc<Q, T, true>(acc, c0, gpx, gpy, gpz, lap);
+            Moments<Q, T, true> m;
+            m.compute(gp);
+            const HydroCell<T> hc = hydro_velocity<T, Q, HVAR>(m, c0, gpx, gpy, gpz, lap, uox, uoy, uoz, a.h);
+            a.Uout[idx] = hc.ux; a.Uout[N + idx] = hc.uy; a.Uout[2 * N + idx] = hc.uz;
+            const Coeffs<T> k = hydro_coeffs<T, Q, HVAR>(m, hc, a.h);
+            T* o = a.Kdst + idx;
+            o[0] = k.A; o[N] = k.bx; o[2 * N] = k.by; o[3 * N] = k.bz;
+            o[4 * N] = k.Txx; o[5 * N] = k.Tyy; o[6 * N] = k.Tzz; o[7 * N] = k.Txy; o[8 * N] = k.Txz; o[9 * N] = k.Tyz;
+        }
+        if constexpr (RING != 4) {
+            __syncthreads();      // everyone is done with the slot of z-1: the plane z+2 takes it
+            if (z + 2 <= ms.ze) ms.load_plane(s + ms.slot_of(z + 2) * NF * TL::TILE, base, g, z + 2);
+            cp_async_commit();
+        }
     }
 }
 
@@ -600,16 +633,33 @@ cudaError_t launch_phase_mom_march(int Q, bool walls, int zchunk, cudaStream_t s
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 
+template <typename T, int Q, bool WALLS, int HVAR, int TX, int TY, int RING, int MINB>
+static cudaError_t launch_hydro_mom_march_v(int zchunk, cudaStream_t stream, const MomHydroArgs<T>& a)
+{
+    using TL = MomTile<TX, TY, RING>;
+    const size_t bytes = (size_t)RING * 11 * TL::TILE * sizeof(T);
+    const Geom& g = a.h.g;
+    const int planes = g.lz1 - g.lz0;
+    const dim3 grid((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (planes + zchunk - 1) / zchunk);
+    auto k = hydro_mom_march_kernel<T, Q, WALLS, HVAR, TX, TY, RING, MINB>;
+    cudaError_t e = march_smem(k, bytes);
+    if (e == cudaSuccess) k<<<grid, dim3(TX, TY, 1), bytes, stream>>>(a, zchunk);
+    return e != cudaSuccess ? e : cudaGetLastError();
+}
+
 template <typename T, int Q, bool WALLS>
 static cudaError_t launch_hydro_mom_march_q(int zchunk, cudaStream_t stream, const MomHydroArgs<T>& a)
 {
-    using TL = MomTile<MARCH_TX, MARCH_TY>;
-    const size_t bytes = (size_t)TL::RING * 10 * TL::TILE * sizeof(T);
-    const Launch l = march_launch(a.h.g, zchunk, stream);
-    cudaError_t e;
-    if (a.h.bulk_one || a.h.subiter > 1) { auto k = hydro_mom_march_kernel<T, Q, WALLS, 1, MARCH_TX, MARCH_TY>; e = march_smem(k, bytes); if (e == cudaSuccess) k<<<l.grid, l.block, bytes, l.stream>>>(a, zchunk); }
-    else { auto k = hydro_mom_march_kernel<T, Q, WALLS, 0, MARCH_TX, MARCH_TY>; e = march_smem(k, bytes); if (e == cudaSuccess) k<<<l.grid, l.block, bytes, l.stream>>>(a, zchunk); }
-    return e != cudaSuccess ? e : cudaGetLastError();
+    const bool var = a.h.bulk_one || a.h.subiter > 1;
+#ifdef ACM_MARCH_PROBE
+    static const int g_march_shape = getenv("ACM_MARCH_SHAPE") ? atoi(getenv("ACM_MARCH_SHAPE")) : 0;
+    if (!var && g_march_shape == 1) return launch_hydro_mom_march_v<T, Q, WALLS, 0, 32, 7, 4, 2>(zchunk, stream, a);
+    if (!var && g_march_shape == 2) return launch_hydro_mom_march_v<T, Q, WALLS, 0, 32, 6, 4, 2>(zchunk, stream, a);
+    if (!var && g_march_shape == 3) return launch_hydro_mom_march_v<T, Q, WALLS, 0, 32, 4, 3, 4>(zchunk, stream, a);
+    if (!var && g_march_shape == 4) return launch_hydro_mom_march_v<T, Q, WALLS, 0, 32, 5, 4, 2>(zchunk, stream, a);
+#endif
+    if (var) return launch_hydro_mom_march_v<T, Q, WALLS, 1, MARCH_TX, MARCH_TY, 3, 2>(zchunk, stream, a);
+    return launch_hydro_mom_march_v<T, Q, WALLS, 0, MARCH_TX, MARCH_TY, 3, 2>(zchunk, stream, a);
 }
 
 template <typename T>
