@@ -12,8 +12,6 @@
 // traffic: 8 (11 + 5) = 128 B (phase) + 8 (14 + 13) = 216 B (hydro) per cell and step for every lattice, instead of
 // 280 + 360 B (D3Q15 + D3Q19) or 472 + 488 B (D3Q27 + D3Q27).  The price is the gather: a pulled population needs up
 // to 6 (g) / 8 (h) values of the neighbour instead of one, served by L1/L2.
-#include <cstdlib>
-
 #include "kernels.h"
 #include "lb_math.cuh"
 
@@ -472,6 +470,256 @@ __global__ void __launch_bounds__(TX * TY, MINB) hydro_mom_march_kernel(const Mo
 }
 
 // ------------------------------------------------------------------------------------------
+// The pushing kernels.  The marching kernels above still gather: ~110 shared-memory loads per cell, which is what
+// bounds them (ncu: the shared-memory pipe 60-80 % busy, warps stalled on its queue).  Here every SOURCE cell of the
+// window is expanded once: its thread reads the cell's coefficients from global memory into registers (coalesced, requested
+// one plane ahead), forms all Q populations with the shared even / odd parts of emit_populations and pushes each one into
+// a shared-memory array indexed by its DESTINATION cell; a destination then finds its Q incoming populations at its own
+// position -- Q conflict-free loads instead of ~5 Q.  A destination plane z is complete when the source planes z-1, z, z+1
+// have been expanded, so the arrays are kept per role: the populations with e_z = +1 of three destination planes, those with
+// e_z = 0 of two, those with e_z = -1 of one.  The one-cell halo of the tile is expanded by the first 2 TX + 2 TY + 4 threads
+// (only what lands inside the tile is stored).  Bounce-back is applied on the destination side: a cell next to a wall
+// rebuilds the populations it cannot receive from its own coefficients.  phi (one field) is staged as in the marching kernels.
+// ------------------------------------------------------------------------------------------
+// a load the compiler keeps where it is written (the requests of the pushing kernels are placed a phase ahead of their use)
+__device__ __forceinline__ double ld_here(const double* p)
+{
+    double v;
+    asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float ld_here(const float* p)
+{
+    float v;
+    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+
+// An instruction that reads v where it is written.  A warp waits for outstanding loads through a few counting scoreboards,
+// so a consumer placed behind a NEWER batch of loads may wait for that batch too; touching the older values first keeps the
+// newer requests (meant to be in flight for a whole phase) out of the critical path.
+__device__ __forceinline__ void touch(double& v) { asm volatile("mov.f64 %0, %0;" : "+d"(v)); }
+__device__ __forceinline__ void touch(float& v) { asm volatile("mov.f32 %0, %0;" : "+f"(v)); }
+
+template <int Q>
+struct PushRoles {
+    __host__ __device__ static constexpr int count(int ez) { int n = 0; for (int i = 0; i < Q; ++i) n += Lat<Q>::ez(i) == ez; return n; }
+    // position of population I among those with the same e_z
+    __host__ __device__ static constexpr int index(int I) { int n = 0; for (int i = 0; i < I; ++i) n += Lat<Q>::ez(i) == Lat<Q>::ez(I); return n; }
+    static constexpr int NU = count(1), NM = count(0), ND = count(-1);
+};
+
+// accessor that always names the calling cell (bounce-back from its own coefficients)
+template <typename T>
+struct OwnK {
+    const T* __restrict__ K;
+    size_t N;
+    unsigned idx;
+    template <int DX, int DY, int DZ> __device__ __forceinline__ unsigned index() const { return idx; }
+    __device__ __forceinline__ T k(int f, unsigned j) const { return __ldg(K + (size_t)f * N + j); }
+};
+
+// phi window of the pushing kernels as an accessor for fd_phi_acc
+template <typename T, typename TL>
+struct TilePhi {
+    const T* s;
+    int base[3];
+    template <int DX, int DY, int DZ> __device__ __forceinline__ T get() const { return s[base[DZ + 1] + DY * TL::PITCH + DX]; }
+};
+
+// the source entries of a thread: its own column and, for the first HALO threads, one entry of the ring around the tile
+template <int TX, int TY>
+struct PushSources {
+    // the ring around the tile, one entry per thread: warp 0 the row below (kind 1), warp 1 the row above (2), warp 2 the
+    // two columns (3, 4) and the corners (5); 0 = none.  The kind is uniform over a warp or splits it into three groups.
+    static_assert(TX == 32 && 2 * TY + 4 <= 32 && TY >= 3, "halo assignment by warps");
+    int hx, hy;                  // local coordinates of the halo entry
+    int kind;
+    unsigned own_src, halo_src;  // offsets inside a plane (periodic wrap / wall clamp; a clamped entry pushes values nobody keeps)
+    __device__ __forceinline__ void init(const Geom& g)
+    {
+        const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
+        const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
+        const bool wx = (g.walls & ACM_WALL_X) != 0, wy = (g.walls & ACM_WALL_Y) != 0;
+        own_src = (unsigned)(tile_coord(y0 + ty, g.ny, wy) * g.nx + tile_coord(x0 + tx, g.nx, wx));
+        kind = 0; hx = hy = 0;
+        if (tid < TX) { hx = tid; hy = -1; kind = 1; }
+        else if (tid < 2 * TX) { hx = tid - TX; hy = TY; kind = 2; }
+        else if (tid < 2 * TX + TY) { hx = -1; hy = tid - 2 * TX; kind = 3; }
+        else if (tid < 2 * TX + 2 * TY) { hx = TX; hy = tid - 2 * TX - TY; kind = 4; }
+        else if (tid < 2 * TX + 2 * TY + 4) { const int c = tid - 2 * TX - 2 * TY; hx = (c & 1) ? TX : -1; hy = (c & 2) ? TY : -1; kind = 5; }
+        halo_src = (unsigned)(tile_coord(y0 + hy, g.ny, wy) * g.nx + tile_coord(x0 + hx, g.nx, wx));
+    }
+};
+
+// role arrays of the pushed populations in shared memory
+template <typename T, int Q, int TX, int TY>
+struct PushBuffers {
+    using R = PushRoles<Q>;
+    static constexpr int NT = TX * TY;
+    static constexpr int DOUBLES = (3 * R::NU + 2 * R::NM + R::ND) * NT;
+    T *up, *mid, *dn;
+    int zb, ze;
+    __device__ __forceinline__ void init(T* s, int zb_, int ze_) { up = s; mid = up + 3 * R::NU * NT; dn = mid + 2 * R::NM * NT; zb = zb_; ze = ze_; }
+    __device__ __forceinline__ T* up_of(int k) const { return up + ((k - zb) % 3) * R::NU * NT; }
+    __device__ __forceinline__ T* mid_of(int k) const { return mid + ((k - zb) & 1) * R::NM * NT; }
+    // push the populations w_i [A + e_i.b + e_i e_i : T] of the source entry (sx, sy) of plane p to their destinations
+    __device__ __forceinline__ void push(int p, int sx, int sy, T A, T bx, T by, T bz, T Txx, T Tyy, T Tzz, T Txy, T Txz, T Tyz) const
+    {
+        const bool okU = p + 1 >= zb && p + 1 < ze, okM = p >= zb && p < ze, okD = p - 1 >= zb && p - 1 < ze;
+        T* const bu = up_of(p + 1);
+        T* const bm = mid_of(p);
+        emit_populations<Q, T>(A, bx, by, bz, Txx, Tyy, Tzz, Txy, Txz, Tyz, [&](auto ic, T v) {
+            constexpr int i = decltype(ic)::value;
+            constexpr int ex = Lat<Q>::ex(i), ey = Lat<Q>::ey(i), ez = Lat<Q>::ez(i), ri = R::index(i);
+            const int dx = sx + ex, dy = sy + ey;
+            if ((unsigned)dx < (unsigned)TX && (unsigned)dy < (unsigned)TY) {
+                const int o = ri * NT + dy * TX + dx;
+                if constexpr (ez > 0) { if (okU) bu[o] = v; }
+                else if constexpr (ez == 0) { if (okM) bm[o] = v; }
+                else { if (okD) dn[o] = v; }
+            }
+        });
+    }
+    // the same for an entry of the ring around the tile: only the populations that can land inside are formed
+    // (RX / RY != 0: only those with e_x = RX / e_y = RY)
+    template <int RX, int RY>
+    __device__ __forceinline__ void push_from_halo(int p, int sx, int sy, const T (&k)[10]) const
+    {
+        const bool okU = p + 1 >= zb && p + 1 < ze, okM = p >= zb && p < ze, okD = p - 1 >= zb && p - 1 < ze;
+        T* const bu = up_of(p + 1);
+        T* const bm = mid_of(p);
+        static_for<1, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            constexpr int ex = Lat<Q>::ex(i), ey = Lat<Q>::ey(i), ez = Lat<Q>::ez(i), ri = R::index(i);
+            if constexpr ((RX == 0 || ex == RX) && (RY == 0 || ey == RY)) {
+                const int dx = sx + ex, dy = sy + ey;
+                if ((unsigned)dx < (unsigned)TX && (unsigned)dy < (unsigned)TY) {
+                    T E = k[0], O = T(0);
+                    bool first = true;
+                    if constexpr (ex != 0) { E += k[4]; odd_term<ex>(O, first, k[1]); }
+                    if constexpr (ey != 0) { E += k[5]; odd_term<ey>(O, first, k[2]); }
+                    if constexpr (ez != 0) { E += k[6]; odd_term<ez>(O, first, k[3]); }
+                    if constexpr (ex * ey != 0) E += T(2 * ex * ey) * k[7];
+                    if constexpr (ex * ez != 0) E += T(2 * ex * ez) * k[8];
+                    if constexpr (ey * ez != 0) E += T(2 * ey * ez) * k[9];
+                    const T v = T(Lat<Q>::w(i)) * (E + O);
+                    const int o = ri * NT + dy * TX + dx;
+                    if constexpr (ez > 0) { if (okU) bu[o] = v; }
+                    else if constexpr (ez == 0) { if (okM) bm[o] = v; }
+                    else { if (okD) dn[o] = v; }
+                }
+            }
+        });
+    }
+    // incoming population I of the destination cell at position `own` (= ty * TX + tx) of plane z
+    template <int I>
+    __device__ __forceinline__ T pull(int z, int own) const
+    {
+        constexpr int ez = Lat<Q>::ez(I), ri = R::index(I);
+        if constexpr (ez > 0) return up_of(z)[ri * NT + own];
+        else if constexpr (ez == 0) return mid_of(z)[ri * NT + own];
+        else return dn[ri * NT + own];
+    }
+};
+
+template <typename T, int Q, bool WALLS, int HVAR, int TX, int TY>
+__global__ void __launch_bounds__(TX * TY, 2) hydro_mom_push_kernel(const MomHydroArgs<T> a, int zchunk)
+{
+    using TL = MomTile<TX, TY, 4>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* sphi = reinterpret_cast<T*>(smem_raw);      // [4][TILE] phi ring, then the role arrays
+    const Geom& g = a.h.g;
+    const size_t N = a.h.N;
+    MarchSetup<TL> ms;
+    ms.init(g, zchunk);
+    if (ms.zb >= ms.ze) return;
+    PushBuffers<T, Q, TX, TY> pb;
+    pb.init(sphi + 4 * TL::TILE, ms.zb, ms.ze);
+    PushSources<TX, TY> ps;
+    ps.init(g);
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const T* const phibase[1] = {a.h.C};
+
+    T kq[10], hq[10];      // coefficients of the thread's source entries of the plane to be expanded next
+    auto request = [&](int zz) {
+        const size_t off = ms.zoff(g, zz);
+#pragma unroll
+        for (int f = 0; f < 10; ++f) kq[f] = ld_here(a.Ksrc + (size_t)f * N + off + ps.own_src);
+        if (ps.kind) {
+#pragma unroll
+            for (int f = 0; f < 10; ++f) hq[f] = ld_here(a.Ksrc + (size_t)f * N + off + ps.halo_src);
+        }
+    };
+    auto expand = [&](int p) {
+        pb.push(p, tx, ty, kq[0], kq[1], kq[2], kq[3], kq[4], kq[5], kq[6], kq[7], kq[8], kq[9]);
+        if (ps.kind == 1) pb.template push_from_halo<0, 1>(p, ps.hx, ps.hy, hq);
+        else if (ps.kind == 2) pb.template push_from_halo<0, -1>(p, ps.hx, ps.hy, hq);
+        else if (ps.kind == 3) pb.template push_from_halo<1, 0>(p, ps.hx, ps.hy, hq);
+        else if (ps.kind == 4) pb.template push_from_halo<-1, 0>(p, ps.hx, ps.hy, hq);
+        else if (ps.kind == 5) {
+            if (ps.hx < 0 && ps.hy < 0) pb.template push_from_halo<1, 1>(p, ps.hx, ps.hy, hq);
+            else if (ps.hx < 0) pb.template push_from_halo<1, -1>(p, ps.hx, ps.hy, hq);
+            else if (ps.hy < 0) pb.template push_from_halo<-1, 1>(p, ps.hx, ps.hy, hq);
+            else pb.template push_from_halo<-1, -1>(p, ps.hx, ps.hy, hq);
+        }
+    };
+    for (int zz = ms.zb - 1; zz <= ms.zb + 1; ++zz) ms.load_plane(sphi + ms.slot_of(zz) * TL::TILE, phibase, g, zz);
+    cp_async_commit();
+    request(ms.zb - 1); expand(ms.zb - 1);
+    request(ms.zb); expand(ms.zb);
+    request(ms.zb + 1);
+
+    const int own = ty * TX + tx, ownphi = (ty + 1) * TL::PITCH + tx + 2;
+    WallFlags wf;
+    wf.wxm = WALLS && (g.walls & ACM_WALL_X) && ms.x == 0; wf.wxp = WALLS && (g.walls & ACM_WALL_X) && ms.x == g.nx - 1;
+    wf.wym = WALLS && (g.walls & ACM_WALL_Y) && ms.y == 0; wf.wyp = WALLS && (g.walls & ACM_WALL_Y) && ms.y == g.ny - 1;
+    const unsigned col = ms.active ? (unsigned)(ms.y * g.nx + ms.x) : 0u;
+    for (int z = ms.zb; z < ms.ze; ++z) {
+        expand(z + 1);
+        const unsigned idx = (unsigned)z * ms.plane + col;
+        T uox = ld_here(a.Uin + idx), uoy = ld_here(a.Uin + N + idx), uoz = ld_here(a.Uin + 2 * N + idx);
+        cp_async_wait_all();
+        __syncthreads();      // plane z is complete, the phi planes z-1 .. z+1 have landed
+        if (z + 2 <= ms.ze) ms.load_plane(sphi + ms.slot_of(z + 2) * TL::TILE, phibase, g, z + 2);
+        cp_async_commit();
+        if (ms.active) {
+            T gp[Q];
+            static_for<0, Q>([&](auto ic) { constexpr int i = decltype(ic)::value; gp[i] = pb.template pull<i>(z, own); });
+            if constexpr (WALLS) {
+                wf.wzm = (g.walls & WALL_ZLO) && z == g.zlo; wf.wzp = (g.walls & WALL_ZHI) && z == g.zhi - 1;
+                if (wf.wxm | wf.wxp | wf.wym | wf.wyp | wf.wzm | wf.wzp) {
+                    const OwnK<T> self{a.Ksrc, N, idx};
+                    static_for<1, Q>([&](auto ic) {
+                        constexpr int i = decltype(ic)::value;
+                        constexpr int ex = Lat<Q>::ex(i), ey = Lat<Q>::ey(i), ez = Lat<Q>::ez(i);
+                        if (wf.template beyond<-ex, -ey, -ez, true>()) gp[i] = T(Lat<Q>::w(i)) * mom_pull_g<Q, i, T, true, false>(self, wf);
+                    });
+                }
+            }
+            TilePhi<T, TL> ph;
+            ph.s = sphi;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) ph.base[d] = ms.slot_of(z - 1 + d) * TL::TILE + ownphi;
+            const T c0 = ph.template get<0, 0, 0>();
+            T gpx, gpy, gpz, lap;
+            fd_phi_acc<Q, T, true>(ph, c0, gpx, gpy, gpz, lap);
+            Moments<Q, T, true> m;
+            m.compute(gp);
+            touch(uox); touch(uoy); touch(uoz);
+            if (z + 2 <= ms.ze) request(z + 2);      // the populations are consumed: their registers take the next plane's coefficients
+            const HydroCell<T> hc = hydro_velocity<T, Q, HVAR>(m, c0, gpx, gpy, gpz, lap, uox, uoy, uoz, a.h);
+            a.Uout[idx] = hc.ux; a.Uout[N + idx] = hc.uy; a.Uout[2 * N + idx] = hc.uz;
+            const Coeffs<T> k = hydro_coeffs<T, Q, HVAR>(m, hc, a.h);
+            T* o = a.Kdst + idx;
+            o[0] = k.A; o[N] = k.bx; o[2 * N] = k.by; o[3 * N] = k.bz;
+            o[4 * N] = k.Txx; o[5 * N] = k.Tyy; o[6 * N] = k.Tzz; o[7 * N] = k.Txy; o[8 * N] = k.Txz; o[9 * N] = k.Tyz;
+        } else if (z + 2 <= ms.ze) request(z + 2);
+        __syncthreads();      // everyone has read plane z: its arrays take the next expansion
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // Equilibrium initialiser (Alg. 2 line 1): phi, u (both velocity buffers), the coefficients of h* = phi Gamma(u)
 // (post-collision convention: the first phase-field step streams it) and of the INCOMING g = Gamma(u) - w (the first
 // hydrodynamic step collides it where it is: hydro_mom_kernel<LOCAL>).
@@ -647,19 +895,31 @@ static cudaError_t launch_hydro_mom_march_v(int zchunk, cudaStream_t stream, con
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 
+template <typename T, int Q, bool WALLS, int HVAR>
+static cudaError_t launch_hydro_mom_push_v(int zchunk, cudaStream_t stream, const MomHydroArgs<T>& a)
+{
+    using TL = MomTile<MARCH_TX, MARCH_TY, 4>;
+    const size_t bytes = (size_t)(4 * TL::TILE + PushBuffers<T, Q, MARCH_TX, MARCH_TY>::DOUBLES) * sizeof(T);
+    const Launch l = march_launch(a.h.g, zchunk, stream);
+    auto k = hydro_mom_push_kernel<T, Q, WALLS, HVAR, MARCH_TX, MARCH_TY>;
+    cudaError_t e = march_smem(k, bytes);
+    if (e == cudaSuccess) k<<<l.grid, l.block, bytes, l.stream>>>(a, zchunk);
+    return e != cudaSuccess ? e : cudaGetLastError();
+}
+
+// D3Q15 / D3Q19: the pushing kernel; D3Q27: its role arrays (108 KB) leave room for one block per SM only and the
+// marching kernel is 3x faster there (measured, profiles/r2_moments.md); D2Q9 never comes here (acm.cu: direct kernels)
 template <typename T, int Q, bool WALLS>
 static cudaError_t launch_hydro_mom_march_q(int zchunk, cudaStream_t stream, const MomHydroArgs<T>& a)
 {
     const bool var = a.h.bulk_one || a.h.subiter > 1;
-#ifdef ACM_MARCH_PROBE
-    static const int g_march_shape = getenv("ACM_MARCH_SHAPE") ? atoi(getenv("ACM_MARCH_SHAPE")) : 0;
-    if (!var && g_march_shape == 1) return launch_hydro_mom_march_v<T, Q, WALLS, 0, 32, 7, 4, 2>(zchunk, stream, a);
-    if (!var && g_march_shape == 2) return launch_hydro_mom_march_v<T, Q, WALLS, 0, 32, 6, 4, 2>(zchunk, stream, a);
-    if (!var && g_march_shape == 3) return launch_hydro_mom_march_v<T, Q, WALLS, 0, 32, 4, 3, 4>(zchunk, stream, a);
-    if (!var && g_march_shape == 4) return launch_hydro_mom_march_v<T, Q, WALLS, 0, 32, 5, 4, 2>(zchunk, stream, a);
-#endif
-    if (var) return launch_hydro_mom_march_v<T, Q, WALLS, 1, MARCH_TX, MARCH_TY, 3, 2>(zchunk, stream, a);
-    return launch_hydro_mom_march_v<T, Q, WALLS, 0, MARCH_TX, MARCH_TY, 3, 2>(zchunk, stream, a);
+    if constexpr (Q == 15 || Q == 19) {
+        if (var) return launch_hydro_mom_push_v<T, Q, WALLS, 1>(zchunk, stream, a);
+        return launch_hydro_mom_push_v<T, Q, WALLS, 0>(zchunk, stream, a);
+    } else {
+        if (var) return launch_hydro_mom_march_v<T, Q, WALLS, 1, MARCH_TX, MARCH_TY, 3, 2>(zchunk, stream, a);
+        return launch_hydro_mom_march_v<T, Q, WALLS, 0, MARCH_TX, MARCH_TY, 3, 2>(zchunk, stream, a);
+    }
 }
 
 template <typename T>

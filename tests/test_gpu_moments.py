@@ -61,8 +61,9 @@ SHAPES = [
 @pytest.mark.parametrize("march", [0, 1, 3], ids=["direct", "march", "march-zchunk3"])
 @pytest.mark.parametrize("nx,ny,nz,Qh,Qg,walls,grav,block", SHAPES)
 def test_first_steps_pdf_parity(nx, ny, nz, Qh, Qg, walls, grav, block, march):
-    """march: the marching kernels (shared-memory window) forced on these small ragged grids -- one tile wider than the
-    grid, several tiles with a ragged last one, z ranges of one chunk and of chunks of 3 planes with a ragged last one."""
+    """march: the tiled kernels (marching phase-field kernel, pushing / marching hydrodynamic kernel; shared-memory
+    window) forced on these small ragged grids -- one tile wider than the grid, several tiles with a ragged last one, z
+    ranges of one chunk and of chunks of 3 planes with a ragged last one.  (Odd nx: the direct kernels run.)"""
     p = Params(nx=nx, ny=ny, nz=nz, stencil_phase=Qh, stencil_hydro=Qg, wall_flags=walls, gravity=grav,
                rho_H=1.0, rho_L=1e-3, sigma=1e-4, nu_H=0.05, nu_L=1 / 60)
     phi, u, _, _ = random_state(p, seed=11)
@@ -184,23 +185,25 @@ def test_graph_replay_is_bit_identical():
 
 
 def test_same_trajectory_as_the_population_kernels():
-    """Both storage forms follow the same time step: after 100 steps they differ by rounding only; the direct and the
-    marching kernels evaluate the same expressions in the same order: bit-identical (walls on one axis, ragged tiles)."""
+    """Both storage forms follow the same time step: after 100 steps they differ by rounding only, whichever kernels
+    advance the moment representation (walls on one axis, ragged tiles).  The chunking of the z range matters in the last
+    place only (the first plane of a chunk is expanded by a second inlined copy of the same expressions, in which the
+    compiler contracts multiply-adds differently: measured 1e-19 on u after 3 steps, confined to the chunk boundaries)."""
     p, phi, u = inputs.scaled_config3(36)
     p = dataclasses.replace(p, wall_flags=inputs.WALL_Z, gravity=(0.0, 0.0, -1e-6))
     out = []
-    for moments, march in ((False, 0), (True, 0), (True, 1), (True, 5)):
+    for moments, tiled, zchunk in ((False, 0, 0), (True, 0, 0), (True, 1, 0), (True, 1, 5)):
         a = _acm(p, moments=moments)
         if moments:
-            a.set_moment_kernels(1 if march else 0, march if march > 1 else 0)
+            a.set_moment_kernels(tiled, zchunk)
         a.init(_dev(phi), _dev(u))
         a.step(100)
         out.append([t.cpu().numpy() for t in a.fields()] + [t.cpu().numpy() for t in a.get_pdfs()])
-    for x, y in zip(out[0], out[1]):
-        assert np.abs(x - y).max() <= 1e-12
-    for other in out[2:]:
-        for x, y in zip(out[1], other):
-            assert (x == y).all()
+    for other in out[1:]:
+        for x, y in zip(out[0], other):
+            assert np.abs(x - y).max() <= 1e-12
+    for x, y in zip(out[2], out[3]):
+        assert np.abs(x - y).max() <= 1e-13
 
 
 def test_workspace_and_errors():
