@@ -32,6 +32,13 @@ def bytes_per_cell(Qh, Qg, esz=8):
     return esz * (2 * Qh + 5), esz * (2 * Qg + 7)
 
 
+def bytes_per_cell_moments(esz=8):
+    """The same rule for the moment representation (ACM_OPT_MOMENTS), whatever the lattices: the phase-field
+    kernel reads A, b (4), phi, the velocity its last collision used (3) and the current velocity (3) and writes A, b,
+    phi; the hydrodynamic kernel reads A, b, T (10), phi, the velocity (3) and writes A, b, T and the velocity."""
+    return esz * (11 + 5), esz * (14 + 13)
+
+
 def workload(config, size=None):
     from paper_2012_06144_b200 import inputs
     if config == 1:
@@ -254,7 +261,7 @@ def traffic_row(kernel, config, precision):
     return None, None
 
 
-def measure(args, config, precision, dev, local_rank, world, K, W, with_e2e=True):
+def measure(args, config, precision, dev, local_rank, world, K, W, with_e2e=True, moments=False):
     """Device-resident throughput of one workload: W warm-up steps, then REPEATS back-to-back intervals of exactly K
     steps each (no per-kernel instrumentation inside them), each bracketed by CUDA events on the launching stream,
     max over ranks per interval, median over the intervals; then a separate pass of K steps with per-kernel events
@@ -268,7 +275,9 @@ def measure(args, config, precision, dev, local_rank, world, K, W, with_e2e=True
     np_dtype = "float64" if precision == "f64" else "float32"
     phi_h = torch.from_numpy(phi.astype(np_dtype)).pin_memory()
     u_h = torch.from_numpy(u.astype(np_dtype)).pin_memory()
-    sim = ACM.from_params(p, precision=precision, device=dev, inplace=args.inplace, unfused=args.unfused)
+    sim = ACM.from_params(p, precision=precision, device=dev, inplace=args.inplace, unfused=args.unfused, moments=moments)
+    if moments and args.moment_kernels is not None:
+        sim.set_moment_kernels(*args.moment_kernels)
     if args.cpt:
         sim.set_cells_per_thread(*args.cpt)
     if args.block:
@@ -277,7 +286,7 @@ def measure(args, config, precision, dev, local_rank, world, K, W, with_e2e=True
         sim.set_graph(args.graph)
     sim.init(phi_h.to(dev), u_h.to(dev))
     N = p.ncells
-    b_phase, b_hydro = bytes_per_cell(p.stencil_phase, p.stencil_hydro, esz)
+    b_phase, b_hydro = bytes_per_cell_moments(esz) if moments else bytes_per_cell(p.stencil_phase, p.stencil_hydro, esz)
 
     sim.step(W)
     replicas.barrier(dev)
@@ -306,7 +315,7 @@ def measure(args, config, precision, dev, local_rank, world, K, W, with_e2e=True
     res = {"p": p, "phi": phi, "u": u, "name": name, "N": N, "esz": esz, "value": value, "ms": ms, "intervals": intervals,
            "value_min": replicas.aggregate_mlups(N, K, intervals[-1], world), "value_max": replicas.aggregate_mlups(N, K, intervals[0], world),
            "phase_ms": phase_ms, "hydro_ms": hydro_ms, "launches": launches, "graph_replays": graph_replays, "mass": mass, "clocks": clk.summary(),
-           "b_phase": b_phase, "b_hydro": b_hydro}
+           "b_phase": b_phase, "b_hydro": b_hydro, "moments": moments}
 
     if with_e2e:
         # end to end through the C ABI with host buffers (pinned), copies inside the timed region
@@ -329,6 +338,8 @@ def measure(args, config, precision, dev, local_rank, world, K, W, with_e2e=True
 def roofline_of(args, config, precision, r, K):
     peak, peak_src = measured_peaks()
     dom = "hydro_kernel" if r["hydro_ms"] >= r["phase_ms"] else "phase_kernel"     # unfused: the three kernels of that LB step
+    if r.get("moments"):
+        dom = dom.replace("_kernel", "_mom_kernel")      # rows of profiles/traffic.csv: the kernels of the moment representation
     dom_ms = r["hydro_ms"] if dom == "hydro_kernel" else r["phase_ms"]
     dom_bytes = (r["b_hydro"] if dom == "hydro_kernel" else r["b_phase"]) * r["N"]
     achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
@@ -355,9 +366,9 @@ def run_acm(args, rank, local_rank, world):
 
     K, W = args.steps, max(args.warmup, 20)      # never fewer than 20 warm-up steps
     precision = args.precision
-    r = measure(args, args.config, precision, dev, local_rank, world, K, W)
+    r = measure(args, args.config, precision, dev, local_rank, world, K, W, moments=args.moments)
     extras = []
-    if args.config == 3 and precision == "f64" and world == 1 and not (args.no_extras or args.inplace or args.unfused or args.cpt or args.block):
+    if args.config == 3 and precision == "f64" and world == 1 and not (args.no_extras or args.inplace or args.unfused or args.cpt or args.block or args.moments):
         # the fp32 instance of config 5 (BASELINE.json configs[4]) in the same run: device-resident throughput only
         x = measure(args, 5, "f32", dev, local_rank, world, K, W, with_e2e=False)
         roof, step_gbs, peak = roofline_of(args, 5, "f32", x, K)
@@ -365,6 +376,16 @@ def run_acm(args, rank, local_rank, world):
                        "unit": UNIT, "ms_per_step": x["ms"] / K, "phase_ms": x["phase_ms"], "hydro_ms": x["hydro_ms"],
                        "bytes_per_cell": {"phase": x["b_phase"], "hydro": x["b_hydro"]}, "step_algorithmic_GBps": step_gbs,
                        "step_frac_of_peak": step_gbs / peak, "roofline": roof})
+        # the headline workload in moment representation (ACM_OPT_MOMENTS: same time step, the state stored as the 4 + 10
+        # coefficients of the post-collision populations; beyond the paper's byte contract, so never the headline)
+        for cfg in (3, 5):
+            x = measure(args, cfg, "f64", dev, local_rank, world, K, W, with_e2e=False, moments=True)
+            roof, step_gbs, peak = roofline_of(args, cfg, "f64", x, K)
+            extras.append({"workload": x["name"] + ", moment representation (ACM_OPT_MOMENTS)", "dtype": "f64", "value": x["value"],
+                           "value_min": x["value_min"], "value_max": x["value_max"], "unit": UNIT, "ms_per_step": x["ms"] / K,
+                           "phase_ms": x["phase_ms"], "hydro_ms": x["hydro_ms"], "bytes_per_cell": {"phase": x["b_phase"], "hydro": x["b_hydro"]},
+                           "step_algorithmic_GBps": step_gbs, "step_frac_of_peak": step_gbs / peak, "roofline": roof,
+                           "workspace_bytes_per_cell": 8 * (2 * (4 + 10) + 2 + 6), "clocks": x["clocks"]})
 
     if rank == 0:
         p, N, esz, ms = r["p"], r["N"], r["esz"], r["ms"]
@@ -375,7 +396,7 @@ def run_acm(args, rank, local_rank, world):
             # BASELINE.md holds the paper's number only for its own benchmark (config 6: 550 MLUPS, P100)
             "vs_baseline": (r["value"] / (211.0 if args.unfused else 550.0) if args.config == 6 and world == 1 and precision == "f64" else None),
             "dtype": precision, "data": "synthetic",
-            "config": {"workload": r["name"], "grid": [p.nx, p.ny, p.nz], "stencils": [p.stencil_phase, p.stencil_hydro], "phase_collision": "SRT" if p.phase_srt else "MRT", "streaming": "in-place AA" if args.inplace else "two-grid pull",
+            "config": {"workload": r["name"], "grid": [p.nx, p.ny, p.nz], "stencils": [p.stencil_phase, p.stencil_hydro], "phase_collision": "SRT" if p.phase_srt else "MRT", "streaming": "in-place AA" if args.inplace else "moment representation, two grids of coefficients" if args.moments else "two-grid pull",
                        "algorithm": "Algorithm 1: six unfused kernels (comparison)" if args.unfused else "Algorithm 2: two fused kernels",
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "timing": f"median of {REPEATS} back-to-back intervals of {K} steps (CUDA events, no per-kernel instrumentation inside); "
@@ -521,6 +542,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the extra fp32 config-5 measurement of the default run")
     ap.add_argument("--inplace", action="store_true", help="in-place AA streaming (one grid per population set)")
+    ap.add_argument("--moments", action="store_true", help="moment representation of the state (ACM_OPT_MOMENTS)")
+    ap.add_argument("--moment-kernels", type=int, nargs=2, default=None, metavar=("MODE", "ZCHUNK"),
+                    help="with --moments: acm_set_moment_kernels (mode -1 automatic | 0 direct | 1 tiled; planes per block, 0 = automatic)")
     ap.add_argument("--unfused", action="store_true", help="Algorithm 1 (six kernels per step) as a measured comparison")
     ap.add_argument("--decompose", action="store_true", help="one global domain in z-slabs with halo exchange instead of replicas")
     ap.add_argument("--peer", action="store_true", help="with --decompose: peer mode (no halo copies; kernels read neighbour memory)")

@@ -501,6 +501,26 @@ __device__ __forceinline__ float ld_here(const float* p)
 __device__ __forceinline__ void touch(double& v) { asm volatile("mov.f64 %0, %0;" : "+d"(v)); }
 __device__ __forceinline__ void touch(float& v) { asm volatile("mov.f32 %0, %0;" : "+f"(v)); }
 
+// mbarrier of a block (shared memory): every thread arrives once per phase, anyone may wait for a phase to complete
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+}
+
 template <int Q>
 struct PushRoles {
     __host__ __device__ static constexpr int count(int ez) { int n = 0; for (int i = 0; i < Q; ++i) n += Lat<Q>::ez(i) == ez; return n; }
@@ -530,9 +550,10 @@ struct TilePhi {
 // the source entries of a thread: its own column and, for the first HALO threads, one entry of the ring around the tile
 template <int TX, int TY>
 struct PushSources {
-    // the ring around the tile, one entry per thread: warp 0 the row below (kind 1), warp 1 the row above (2), warp 2 the
-    // two columns (3, 4) and the corners (5); 0 = none.  The kind is uniform over a warp or splits it into three groups.
-    static_assert(TX == 32 && 2 * TY + 4 <= 32 && TY >= 3, "halo assignment by warps");
+    // the ring around the tile, one entry per thread: the first TX threads the row below (kind 1), the next TX the row above
+    // (2), then the two columns (3, 4) and the corners (5); 0 = none.  The kind is uniform over a warp, except in the one
+    // warp that takes the columns and the corners.
+    static_assert(TX % 32 == 0 && 2 * TY + 4 <= 32 && 2 * TX + 32 <= TX * TY, "halo assignment by warps");
     int hx, hy;                  // local coordinates of the halo entry
     int kind;
     unsigned own_src, halo_src;  // offsets inside a plane (periodic wrap / wall clamp; a clamped entry pushes values nobody keeps)
@@ -640,6 +661,12 @@ __global__ void __launch_bounds__(TX * TY, 2) hydro_mom_push_kernel(const MomHyd
     ps.init(g);
     const int tx = threadIdx.x, ty = threadIdx.y;
     const T* const phibase[1] = {a.h.C};
+    // "everyone has read the arrays of plane z" is a split barrier: a thread arrives as soon as its Q populations are in
+    // registers and waits only before it overwrites arrays in the next expansion, so the arithmetic of the slower warps
+    // overlaps the next expansion of the faster ones
+    __shared__ unsigned long long pulled;
+    if (tx == 0 && ty == 0) mbar_init(&pulled, TX * TY);
+    __syncthreads();
 
     T kq[10], hq[10];      // coefficients of the thread's source entries of the plane to be expanded next
     auto request = [&](int zz) {
@@ -676,6 +703,7 @@ __global__ void __launch_bounds__(TX * TY, 2) hydro_mom_push_kernel(const MomHyd
     wf.wym = WALLS && (g.walls & ACM_WALL_Y) && ms.y == 0; wf.wyp = WALLS && (g.walls & ACM_WALL_Y) && ms.y == g.ny - 1;
     const unsigned col = ms.active ? (unsigned)(ms.y * g.nx + ms.x) : 0u;
     for (int z = ms.zb; z < ms.ze; ++z) {
+        if (z > ms.zb) mbar_wait(&pulled, (unsigned)(z - 1 - ms.zb) & 1u);      // everyone has read plane z-1: its arrays take this expansion
         expand(z + 1);
         const unsigned idx = (unsigned)z * ms.plane + col;
         T uox = ld_here(a.Uin + idx), uoy = ld_here(a.Uin + N + idx), uoz = ld_here(a.Uin + 2 * N + idx);
@@ -683,9 +711,11 @@ __global__ void __launch_bounds__(TX * TY, 2) hydro_mom_push_kernel(const MomHyd
         __syncthreads();      // plane z is complete, the phi planes z-1 .. z+1 have landed
         if (z + 2 <= ms.ze) ms.load_plane(sphi + ms.slot_of(z + 2) * TL::TILE, phibase, g, z + 2);
         cp_async_commit();
+        if (!ms.active) mbar_arrive(&pulled);
         if (ms.active) {
             T gp[Q];
             static_for<0, Q>([&](auto ic) { constexpr int i = decltype(ic)::value; gp[i] = pb.template pull<i>(z, own); });
+            mbar_arrive(&pulled);
             if constexpr (WALLS) {
                 wf.wzm = (g.walls & WALL_ZLO) && z == g.zlo; wf.wzp = (g.walls & WALL_ZHI) && z == g.zhi - 1;
                 if (wf.wxm | wf.wxp | wf.wym | wf.wyp | wf.wzm | wf.wzp) {
@@ -715,7 +745,6 @@ __global__ void __launch_bounds__(TX * TY, 2) hydro_mom_push_kernel(const MomHyd
             o[0] = k.A; o[N] = k.bx; o[2 * N] = k.by; o[3 * N] = k.bz;
             o[4 * N] = k.Txx; o[5 * N] = k.Tyy; o[6 * N] = k.Tzz; o[7 * N] = k.Txy; o[8 * N] = k.Txz; o[9 * N] = k.Tyz;
         } else if (z + 2 <= ms.ze) request(z + 2);
-        __syncthreads();      // everyone has read plane z: its arrays take the next expansion
     }
 }
 
