@@ -337,11 +337,12 @@ def measure(args, config, precision, dev, local_rank, world, K, W, with_e2e=True
 
 def roofline_of(args, config, precision, r, K):
     peak, peak_src = measured_peaks()
-    dom = "hydro_kernel" if r["hydro_ms"] >= r["phase_ms"] else "phase_kernel"     # unfused: the three kernels of that LB step
+    hydro = r["hydro_ms"] >= r["phase_ms"]
+    dom = "hydro_kernel" if hydro else "phase_kernel"     # unfused: the three kernels of that LB step
     if r.get("moments"):
         dom = dom.replace("_kernel", "_mom_kernel")      # rows of profiles/traffic.csv: the kernels of the moment representation
-    dom_ms = r["hydro_ms"] if dom == "hydro_kernel" else r["phase_ms"]
-    dom_bytes = (r["b_hydro"] if dom == "hydro_kernel" else r["b_phase"]) * r["N"]
+    dom_ms = r["hydro_ms"] if hydro else r["phase_ms"]
+    dom_bytes = (r["b_hydro"] if hydro else r["b_phase"]) * r["N"]
     achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
     step_gbs = (r["b_phase"] + r["b_hydro"]) * r["N"] * K / (r["ms"] * 1e-3) / 1e9
     traffic, commit = traffic_row(dom, config, precision)

@@ -32,6 +32,13 @@ def test_traffic_table_rows_carry_the_commit_of_their_build():
     t, commit = bench.traffic_row("hydro_kernel", 5, "f32")
     assert commit and 0.95 < t / (244 * 256 ** 3) < 1.05
     assert bench.traffic_row("hydro_kernel", 99, "f64") == (None, None)
+    # moment representation: 128 + 216 B per cell whatever the lattices
+    assert bench.bytes_per_cell_moments() == (128, 216)
+    for cfg in (3, 5):
+        t, commit = bench.traffic_row("hydro_mom_kernel", cfg, "f64")
+        assert commit and 0.95 < t / (216 * 256 ** 3) < 1.05
+        t, commit = bench.traffic_row("phase_mom_kernel", cfg, "f64")
+        assert commit and 0.95 < t / (128 * 256 ** 3) < 1.05
 
 
 def test_roofline_arithmetic():
@@ -48,6 +55,9 @@ def test_roofline_arithmetic():
     assert roof["peak_is_lower_bound"] == (roof["achieved"] > peak)
     assert abs(step_gbs - 640 * N / 1.6e-3 / 1e9) < 1e-6
     assert abs(roof["kernel_share_of_step"] - 0.9 / 1.6) < 1e-12
+    m = {"hydro_ms": 0.9, "phase_ms": 0.62, "b_hydro": 216, "b_phase": 128, "N": N, "ms": 1.52 * 20, "moments": True}
+    roof, step_gbs, peak = bench.roofline_of(args, 3, "f64", m, 20)
+    assert roof["kernel"] == "hydro_mom_kernel" and roof["traffic"] and abs(roof["achieved"] - 216 * N / 0.9e-3 / 1e9) < 1e-6
 
 
 def test_reference_arm_prints_one_json_line():
