@@ -139,12 +139,15 @@ int acm_init(acm_ctx*, const void* phi, const void* u);
 int acm_set_subiter(acm_ctx*, int sweeps);
 
 /* ACM_OPT_MOMENTS only (ACM_ESTATE otherwise): which kernels advance the moment representation.
- *   mode  -1 (default) automatic: the marching kernels for three-dimensional grids of at least 2^21 cells, else the
+ *   mode  -1 (default) automatic: the tiled kernels for three-dimensional grids of at least 2^21 cells, else the
  *            direct ones; 0 = direct kernels (one thread per cell, the coefficients of the neighbours gathered through
- *            L1/L2); 1 = marching kernels (a block owns a 32 x 8 tile of columns and marches along z, the coefficient
- *            planes of the tile and its halo staged in a four-plane shared-memory ring by cp.async).
- *   zchunk planes a block of the marching kernels covers; 0 (default) = chosen such that the blocks fill whole waves.
- * Same results either way (bit-identical: both evaluate the same expressions in the same order).  ACM_EINVAL for other values. */
+ *            L1/L2); 1 = tiled kernels: a block owns a 32 x 8 tile of columns and marches along z with a window of planes
+ *            in shared memory -- the phase-field kernel (and the D3Q27 hydrodynamic kernel) gathers from coefficient
+ *            planes staged by cp.async, the D3Q15 / D3Q19 hydrodynamic kernel expands every source cell once into
+ *            destination-indexed arrays.  Grids with odd nx and the two-dimensional instance always run the direct kernels.
+ *   zchunk planes a block of the tiled kernels covers; 0 (default) = chosen such that the blocks fill whole waves.
+ * Same results up to rounding (the kernels evaluate the same formulas in different association; the chunking matters in
+ * the last place only).  ACM_EINVAL for other values. */
 int acm_set_moment_kernels(acm_ctx*, int mode, int zchunk);
 
 /* ACM_F32 only (no effect for ACM_F64).  The fp32 instance stores h_i - ref w_i and phi - ref instead of h_i and

@@ -11,7 +11,10 @@
 // The trajectory is the one of the population kernels up to rounding (same oracle, same bars); what changes is the
 // traffic: 8 (11 + 5) = 128 B (phase) + 8 (14 + 13) = 216 B (hydro) per cell and step for every lattice, instead of
 // 280 + 360 B (D3Q15 + D3Q19) or 472 + 488 B (D3Q27 + D3Q27).  The price is the gather: a pulled population needs up
-// to 6 (g) / 8 (h) values of the neighbour instead of one, served by L1/L2.
+// to 6 (g) / 8 (h) values of the neighbour instead of one.  Three kernel families, all instances of the same pull /
+// collide functions over an accessor: DIRECT (one thread per cell, gather through L1/L2), MARCHING (tile of columns
+// marching along z, coefficient planes staged in shared memory) and PUSHING (every source cell of the window expanded once
+// into destination-indexed shared-memory arrays).  Measurements and the way there: DESIGN.md 5.10, profiles/r2b_profiles.md.
 #include "kernels.h"
 #include "lb_math.cuh"
 
@@ -937,7 +940,7 @@ static cudaError_t launch_hydro_mom_push_v(int zchunk, cudaStream_t stream, cons
 }
 
 // D3Q15 / D3Q19: the pushing kernel; D3Q27: its role arrays (108 KB) leave room for one block per SM only and the
-// marching kernel is 3x faster there (measured, profiles/r2_moments.md); D2Q9 never comes here (acm.cu: direct kernels)
+// marching kernel is 3x faster there (measured, profiles/r2b_profiles.md section 3); D2Q9 never comes here (acm.cu: direct kernels)
 template <typename T, int Q, bool WALLS>
 static cudaError_t launch_hydro_mom_march_q(int zchunk, cudaStream_t stream, const MomHydroArgs<T>& a)
 {
