@@ -587,21 +587,40 @@ struct PushBuffers {
     __device__ __forceinline__ void init(T* s, int zb_, int ze_) { up = s; mid = up + 3 * R::NU * NT; dn = mid + 2 * R::NM * NT; zb = zb_; ze = ze_; }
     __device__ __forceinline__ T* up_of(int k) const { return up + ((k - zb) % 3) * R::NU * NT; }
     __device__ __forceinline__ T* mid_of(int k) const { return mid + ((k - zb) & 1) * R::NM * NT; }
-    // push the populations w_i [A + e_i.b + e_i e_i : T] of the source entry (sx, sy) of plane p to their destinations
-    __device__ __forceinline__ void push(int p, int sx, int sy, T A, T bx, T by, T bz, T Txx, T Tyy, T Tzz, T Txy, T Txz, T Tyz) const
+    // bit i: population i of the source entry (sx, sy) lands inside the tile (constant along the march)
+    __device__ __forceinline__ static unsigned inside_mask(int sx, int sy)
+    {
+        unsigned m = 0;
+        static_for<0, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            const int dx = sx + Lat<Q>::ex(i), dy = sy + Lat<Q>::ey(i);
+            if ((unsigned)dx < (unsigned)TX && (unsigned)dy < (unsigned)TY) m |= 1u << i;
+        });
+        return m;
+    }
+    __host__ __device__ static constexpr unsigned role_bits(int ez)
+    {
+        unsigned m = 0;
+        for (int i = 0; i < Q; ++i) if (Lat<Q>::ez(i) == ez) m |= 1u << i;
+        return m;
+    }
+    // push the populations w_i [A + e_i.b + e_i e_i : T] of the thread's own source entry (position `own`, mask of the
+    // populations that land inside the tile) of plane p to their destinations: own + a compile-time offset
+    __device__ __forceinline__ void push(int p, int own, unsigned inside, T A, T bx, T by, T bz, T Txx, T Tyy, T Tzz, T Txy, T Txz, T Tyz) const
     {
         const bool okU = p + 1 >= zb && p + 1 < ze, okM = p >= zb && p < ze, okD = p - 1 >= zb && p - 1 < ze;
-        T* const bu = up_of(p + 1);
-        T* const bm = mid_of(p);
+        const unsigned live = inside & ((okU ? role_bits(1) : 0u) | (okM ? role_bits(0) : 0u) | (okD ? role_bits(-1) : 0u));
+        T* const bu = up_of(p + 1) + own;
+        T* const bm = mid_of(p) + own;
+        T* const bd = dn + own;
         emit_populations<Q, T>(A, bx, by, bz, Txx, Tyy, Tzz, Txy, Txz, Tyz, [&](auto ic, T v) {
             constexpr int i = decltype(ic)::value;
             constexpr int ex = Lat<Q>::ex(i), ey = Lat<Q>::ey(i), ez = Lat<Q>::ez(i), ri = R::index(i);
-            const int dx = sx + ex, dy = sy + ey;
-            if ((unsigned)dx < (unsigned)TX && (unsigned)dy < (unsigned)TY) {
-                const int o = ri * NT + dy * TX + dx;
-                if constexpr (ez > 0) { if (okU) bu[o] = v; }
-                else if constexpr (ez == 0) { if (okM) bm[o] = v; }
-                else { if (okD) dn[o] = v; }
+            constexpr int o = ri * NT + ey * TX + ex;
+            if (live & (1u << i)) {
+                if constexpr (ez > 0) bu[o] = v;
+                else if constexpr (ez == 0) bm[o] = v;
+                else bd[o] = v;
             }
         });
     }
@@ -663,6 +682,8 @@ __global__ void __launch_bounds__(TX * TY, 2) hydro_mom_push_kernel(const MomHyd
     PushSources<TX, TY> ps;
     ps.init(g);
     const int tx = threadIdx.x, ty = threadIdx.y;
+    const int own = ty * TX + tx, ownphi = (ty + 1) * TL::PITCH + tx + 2;
+    const unsigned inside = PushBuffers<T, Q, TX, TY>::inside_mask(tx, ty);
     const T* const phibase[1] = {a.h.C};
     // "everyone has read the arrays of plane z" is a split barrier: a thread arrives as soon as its Q populations are in
     // registers and waits only before it overwrites arrays in the next expansion, so the arithmetic of the slower warps
@@ -682,7 +703,7 @@ __global__ void __launch_bounds__(TX * TY, 2) hydro_mom_push_kernel(const MomHyd
         }
     };
     auto expand = [&](int p) {
-        pb.push(p, tx, ty, kq[0], kq[1], kq[2], kq[3], kq[4], kq[5], kq[6], kq[7], kq[8], kq[9]);
+        pb.push(p, own, inside, kq[0], kq[1], kq[2], kq[3], kq[4], kq[5], kq[6], kq[7], kq[8], kq[9]);
         if (ps.kind == 1) pb.template push_from_halo<0, 1>(p, ps.hx, ps.hy, hq);
         else if (ps.kind == 2) pb.template push_from_halo<0, -1>(p, ps.hx, ps.hy, hq);
         else if (ps.kind == 3) pb.template push_from_halo<1, 0>(p, ps.hx, ps.hy, hq);
@@ -700,7 +721,6 @@ __global__ void __launch_bounds__(TX * TY, 2) hydro_mom_push_kernel(const MomHyd
     request(ms.zb); expand(ms.zb);
     request(ms.zb + 1);
 
-    const int own = ty * TX + tx, ownphi = (ty + 1) * TL::PITCH + tx + 2;
     WallFlags wf;
     wf.wxm = WALLS && (g.walls & ACM_WALL_X) && ms.x == 0; wf.wxp = WALLS && (g.walls & ACM_WALL_X) && ms.x == g.nx - 1;
     wf.wym = WALLS && (g.walls & ACM_WALL_Y) && ms.y == 0; wf.wyp = WALLS && (g.walls & ACM_WALL_Y) && ms.y == g.ny - 1;
