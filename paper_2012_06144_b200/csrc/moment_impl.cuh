@@ -498,11 +498,6 @@ __device__ __forceinline__ float ld_here(const float* p)
     return v;
 }
 
-// An instruction that reads v where it is written.  A warp waits for outstanding loads through a few counting scoreboards,
-// so a consumer placed behind a NEWER batch of loads may wait for that batch too; touching the older values first keeps the
-// newer requests (meant to be in flight for a whole phase) out of the critical path.
-__device__ __forceinline__ void touch(double& v) { asm volatile("mov.f64 %0, %0;" : "+d"(v)); }
-__device__ __forceinline__ void touch(float& v) { asm volatile("mov.f32 %0, %0;" : "+f"(v)); }
 
 // mbarrier of a block (shared memory): every thread arrives once per phase, anyone may wait for a phase to complete
 __device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count)
@@ -729,7 +724,7 @@ __global__ void __launch_bounds__(TX * TY, 2) hydro_mom_push_kernel(const MomHyd
         if (z > ms.zb) mbar_wait(&pulled, (unsigned)(z - 1 - ms.zb) & 1u);      // everyone has read plane z-1: its arrays take this expansion
         expand(z + 1);
         const unsigned idx = (unsigned)z * ms.plane + col;
-        T uox = ld_here(a.Uin + idx), uoy = ld_here(a.Uin + N + idx), uoz = ld_here(a.Uin + 2 * N + idx);
+        const T uox = ld_here(a.Uin + idx), uoy = ld_here(a.Uin + N + idx), uoz = ld_here(a.Uin + 2 * N + idx);
         cp_async_wait_all();
         __syncthreads();      // plane z is complete, the phi planes z-1 .. z+1 have landed
         if (z + 2 <= ms.ze) ms.load_plane(sphi + ms.slot_of(z + 2) * TL::TILE, phibase, g, z + 2);
@@ -759,7 +754,6 @@ __global__ void __launch_bounds__(TX * TY, 2) hydro_mom_push_kernel(const MomHyd
             fd_phi_acc<Q, T, true>(ph, c0, gpx, gpy, gpz, lap);
             Moments<Q, T, true> m;
             m.compute(gp);
-            touch(uox); touch(uoy); touch(uoz);
             if (z + 2 <= ms.ze) request(z + 2);      // the populations are consumed: their registers take the next plane's coefficients
             const HydroCell<T> hc = hydro_velocity<T, Q, HVAR>(m, c0, gpx, gpy, gpz, lap, uox, uoy, uoz, a.h);
             a.Uout[idx] = hc.ux; a.Uout[N + idx] = hc.uy; a.Uout[2 * N + idx] = hc.uz;
