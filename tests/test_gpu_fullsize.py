@@ -87,26 +87,29 @@ def _check_one_step_sampled(p, phi, u, starts, presteps=2, **kw):
     return worst
 
 
-def test_config2_full_size_walls_gravity():
+@pytest.mark.parametrize("moments", [False, True], ids=["populations", "moments"])
+def test_config2_full_size_walls_gravity(moments):
     """128 x 512 x 128, half-way bounce-back walls in y, gravity: sub-boxes on both walls, on the
-    bubble's interface (centre (64,64,64), R=16), across the periodic x/z seams."""
+    bubble's interface (centre (64,64,64), R=16), across the periodic x/z seams.  moments: the same in moment
+    representation (ACM_OPT_MOMENTS, tiled kernels; the populations compared are the ones acm_get_pdfs rebuilds)."""
     p, phi, u = inputs.config2()
     starts = [(0, 0, 0), (p.nz - 7, p.ny - B, p.nx - 7), (57, 0, 57), (57, 41, 57), (57, 73, 57), (57, 57, 73),
               (120, 300, 3), (57, p.ny - B, 57)]
     # z, y, x order
-    _check_one_step_sampled(p, phi, u, starts)
+    _check_one_step_sampled(p, phi, u, starts, moments=moments)
 
 
-def test_config5_full_size_q27_fp64():
+@pytest.mark.parametrize("moments", [False, True], ids=["populations", "moments"])
+def test_config5_full_size_q27_fp64(moments):
     """256^3 D3Q27 + D3Q27 fp64 (the fp64 leg of config 5)."""
     p, phi, u = inputs.config5()
     cs, rs = inputs.bubble_set(p, 64, 8.0, 14.0)
     starts = [(0, 0, 0), (p.nz - 7, p.ny - 7, p.nx - 7), (37, 201, 118),
               tuple(int(v) - 7 for v in (cs[3] + np.array([0.0, 0.0, rs[3]]))[::-1])]
-    _check_one_step_sampled(p, phi, u, starts)
+    _check_one_step_sampled(p, phi, u, starts, moments=moments)
 
 
-@pytest.mark.parametrize("inplace", [False, True])
+@pytest.mark.parametrize("inplace", [False, True, "moments"])
 def test_config4_full_size_512(inplace):
     """512^3 (134 M cells, 64-bit plane offsets: the last h plane starts at element 14*2^27): needs
     ~125 GB of the 180 GB for the two-grid layout plus the exported populations."""
@@ -123,4 +126,7 @@ def test_config4_full_size_512(inplace):
               tuple(int(v) - 7 for v in (cs[0] + np.array([rs[0], 0.0, 0.0]))[::-1]),
               tuple(int(v) - 7 for v in (cs[100] + np.array([0.0, -rs[100], 0.0]))[::-1])]
     # the in-place pattern alternates two kernels: 2 pre-steps then an odd..even pair is covered by presteps 2 and 3
-    _check_one_step_sampled(p, phi, u, starts, presteps=3 if inplace else 2, inplace=inplace)
+    if inplace == "moments":      # moment representation: 38.6 GB of workspace instead of 79.5
+        _check_one_step_sampled(p, phi, u, starts, moments=True)
+    else:
+        _check_one_step_sampled(p, phi, u, starts, presteps=3 if inplace else 2, inplace=inplace)
