@@ -240,9 +240,11 @@ __global__ void __launch_bounds__(ACM_MAXT) hydro_mom_kernel(const MomHydroArgs<
 // The marching kernels.  The direct kernels above are latency-bound: each thread issues ~110 dependent-free but
 // register-limited loads per cell through L1 (ncu: DRAM at half its rate, nothing else saturated).  Here a block owns a
 // TX x TY tile of columns and marches along z over `zchunk` planes; the coefficient planes it needs (tile + one-cell
-// halo, periodic wrap / wall clamp applied by the loader) travel global -> shared memory by cp.async into a ring of
-// four plane slots: while plane z is computed from the slots of z-1, z, z+1, plane z+2 is in flight.  One barrier per
-// plane.  Every coefficient is fetched from L2 once per tile (+ halo), the gather runs on shared memory.
+// halo, periodic wrap / wall clamp applied by the loader; phi and -- for the phase-field step -- the velocity staged with
+// them) travel global -> shared memory by cp.async into a ring of plane slots.  Phase-field kernel: four slots, plane z+2
+// is in flight while plane z is computed from the slots of z-1, z, z+1, one barrier per plane.  Hydrodynamic kernel (eleven
+// fields): three slots, so that two blocks fit an SM; plane z+2 is requested after the computation of plane z.  Every
+// coefficient is fetched from L2 once per tile (+ halo), the gather runs on shared memory.
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ void cp_async8(void* smem, const void* gmem)
 {
@@ -408,9 +410,11 @@ __global__ void __launch_bounds__(TX * TY, 2) phase_mom_march_kernel(const MomPh
     }
 }
 
-template <typename T, int Q, bool WALLS, int HVAR, int TX, int TY, int RING, int MINB>
-__global__ void __launch_bounds__(TX * TY, MINB) hydro_mom_march_kernel(const MomHydroArgs<T> a, int zchunk)
+// (ring of 3 plane slots: two blocks per SM; the next plane is requested after the computation and lands under the other block's)
+template <typename T, int Q, bool WALLS, int HVAR, int TX, int TY>
+__global__ void __launch_bounds__(TX * TY, 2) hydro_mom_march_kernel(const MomHydroArgs<T> a, int zchunk)
 {
+    constexpr int RING = 3;
     using TL = MomTile<TX, TY, RING>;
     constexpr int NF = 11;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -436,11 +440,7 @@ __global__ void __launch_bounds__(TX * TY, MINB) hydro_mom_march_kernel(const Mo
         const unsigned idx = (unsigned)z * ms.plane + col;
         const T uox = __ldg(a.Uin + idx), uoy = __ldg(a.Uin + N + idx), uoz = __ldg(a.Uin + 2 * N + idx);
         cp_async_wait_all();
-        __syncthreads();      // planes z-1 .. z+1 have landed for everyone (RING 4: and everyone is done with the slot of z-2)
-        if constexpr (RING == 4) {
-            if (z + 2 <= ms.ze) ms.load_plane(s + ms.slot_of(z + 2) * NF * TL::TILE, base, g, z + 2);
-            cp_async_commit();
-        }
+        __syncthreads();      // planes z-1 .. z+1 have landed for everyone
         if (ms.active) {
             wf.wzm = WALLS && (g.walls & WALL_ZLO) && z == g.zlo; wf.wzp = WALLS && (g.walls & WALL_ZHI) && z == g.zhi - 1;
             TileK<T, TL> acc;
@@ -464,11 +464,9 @@ __global__ void __launch_bounds__(TX * TY, MINB) hydro_mom_march_kernel(const Mo
             o[0] = k.A; o[N] = k.bx; o[2 * N] = k.by; o[3 * N] = k.bz;
             o[4 * N] = k.Txx; o[5 * N] = k.Tyy; o[6 * N] = k.Tzz; o[7 * N] = k.Txy; o[8 * N] = k.Txz; o[9 * N] = k.Tyz;
         }
-        if constexpr (RING != 4) {
-            __syncthreads();      // everyone is done with the slot of z-1: the plane z+2 takes it
-            if (z + 2 <= ms.ze) ms.load_plane(s + ms.slot_of(z + 2) * NF * TL::TILE, base, g, z + 2);
-            cp_async_commit();
-        }
+        __syncthreads();      // everyone is done with the slot of z-1: the plane z+2 takes it
+        if (z + 2 <= ms.ze) ms.load_plane(s + ms.slot_of(z + 2) * NF * TL::TILE, base, g, z + 2);
+        cp_async_commit();
     }
 }
 
@@ -927,17 +925,15 @@ cudaError_t launch_phase_mom_march(int Q, bool walls, int zchunk, cudaStream_t s
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 
-template <typename T, int Q, bool WALLS, int HVAR, int TX, int TY, int RING, int MINB>
+template <typename T, int Q, bool WALLS, int HVAR>
 static cudaError_t launch_hydro_mom_march_v(int zchunk, cudaStream_t stream, const MomHydroArgs<T>& a)
 {
-    using TL = MomTile<TX, TY, RING>;
-    const size_t bytes = (size_t)RING * 11 * TL::TILE * sizeof(T);
-    const Geom& g = a.h.g;
-    const int planes = g.lz1 - g.lz0;
-    const dim3 grid((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (planes + zchunk - 1) / zchunk);
-    auto k = hydro_mom_march_kernel<T, Q, WALLS, HVAR, TX, TY, RING, MINB>;
+    using TL = MomTile<MARCH_TX, MARCH_TY, 3>;
+    const size_t bytes = (size_t)3 * 11 * TL::TILE * sizeof(T);
+    const Launch l = march_launch(a.h.g, zchunk, stream);
+    auto k = hydro_mom_march_kernel<T, Q, WALLS, HVAR, MARCH_TX, MARCH_TY>;
     cudaError_t e = march_smem(k, bytes);
-    if (e == cudaSuccess) k<<<grid, dim3(TX, TY, 1), bytes, stream>>>(a, zchunk);
+    if (e == cudaSuccess) k<<<l.grid, l.block, bytes, l.stream>>>(a, zchunk);
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 
@@ -954,7 +950,7 @@ static cudaError_t launch_hydro_mom_push_v(int zchunk, cudaStream_t stream, cons
 }
 
 // D3Q15 / D3Q19: the pushing kernel; D3Q27: its role arrays (108 KB) leave room for one block per SM only and the
-// marching kernel is 3x faster there (measured, profiles/r2b_profiles.md section 3); D2Q9 never comes here (acm.cu: direct kernels)
+// marching kernel is 3x faster there (measured, profiles/r2b_profiles.md section 3); D2Q9 comes here only when acm_set_moment_kernels forces it (acm.cu: direct kernels by default)
 template <typename T, int Q, bool WALLS>
 static cudaError_t launch_hydro_mom_march_q(int zchunk, cudaStream_t stream, const MomHydroArgs<T>& a)
 {
@@ -963,8 +959,8 @@ static cudaError_t launch_hydro_mom_march_q(int zchunk, cudaStream_t stream, con
         if (var) return launch_hydro_mom_push_v<T, Q, WALLS, 1>(zchunk, stream, a);
         return launch_hydro_mom_push_v<T, Q, WALLS, 0>(zchunk, stream, a);
     } else {
-        if (var) return launch_hydro_mom_march_v<T, Q, WALLS, 1, MARCH_TX, MARCH_TY, 3, 2>(zchunk, stream, a);
-        return launch_hydro_mom_march_v<T, Q, WALLS, 0, MARCH_TX, MARCH_TY, 3, 2>(zchunk, stream, a);
+        if (var) return launch_hydro_mom_march_v<T, Q, WALLS, 1>(zchunk, stream, a);
+        return launch_hydro_mom_march_v<T, Q, WALLS, 0>(zchunk, stream, a);
     }
 }
 
