@@ -258,3 +258,20 @@ def test_config5_fp32_500_steps_against_the_oracle():
         print(f"config 5 fp32 instance vs fp64 oracle, 256^3, step {n}: max|dphi| {dphi:.2e} max|du| {du:.2e}", flush=True)
     assert dphi <= 1e-5 and du <= 1e-5, (dphi, du)
     assert abs(a.phi_mass() - m0) <= 1e-6 * m0
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("ACM_LONG"), reason="about 7 minutes of oracle time: set ACM_LONG=1")
+def test_config5_fp64_100_steps_against_the_oracle():
+    """north_star's 100-step bar on config 5's fp64 leg at full size (256^3 D3Q27 + D3Q27, every element), for the
+    population path and the moment representation.  Opt-in (the oracle needs ~4 s per step here); the run on record is
+    in profiles/r2b_profiles.md section 5."""
+    p, phi, u = inputs.config5()
+    t = _Twin(p, phi, u, with_moments=True)
+    for n in (10, 50, 100):
+        t.advance_to(n)
+        d, m = t.field_diffs(), t.field_diffs("m")
+        print(f"config 5 fp64, 256^3 D3Q27, step {n}: max|dphi| {d[0]:.2e} |du| {d[1]:.2e} |dp| {d[2]:.2e};  "
+              f"moment representation: {m[0]:.2e} {m[1]:.2e} {m[2]:.2e}", flush=True)
+    assert max(d) <= TOL_FIELD_100 and max(m) <= TOL_FIELD_100, (d, m)
+    mass = t.a.phi_mass()
+    assert abs(mass - t.o.phi_mass()) <= 1e-12 * abs(mass) and abs(t.m.phi_mass() - t.o.phi_mass()) <= 1e-12 * abs(mass)
