@@ -245,6 +245,26 @@ def pick_device(local_rank):
     return local_rank, torch.device("cuda", local_rank)
 
 
+def copy_bandwidth(dev, n=1 << 28, repeats=10):
+    """Device-to-device copy of n fp64 values (read + write bytes, best of `repeats`, CUDA events): the box's copy
+    bandwidth re-measured in this run; the roofline's denominator stays MEASURED_PEAKS.json's."""
+    import torch
+    a = torch.empty(n, dtype=torch.float64, device=dev).normal_()
+    b = torch.empty_like(a)
+    b.copy_(a)
+    best = float("inf")
+    for _ in range(repeats):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        b.copy_(a)
+        e1.record()
+        torch.cuda.synchronize(dev)
+        best = min(best, e0.elapsed_time(e1))
+    del a, b
+    torch.cuda.empty_cache()
+    return 2 * n * 8 / (best * 1e-3) / 1e9
+
+
 NOMINAL_HBM_GBS = 8000.0      # vendor figure for context (B200_PROFILING.md: 7.7 TB/s HGX, 8 TB/s DGX)
 REPEATS = 5
 
@@ -368,6 +388,7 @@ def run_acm(args, rank, local_rank, world):
     K, W = args.steps, max(args.warmup, 20)      # never fewer than 20 warm-up steps
     precision = args.precision
     r = measure(args, args.config, precision, dev, local_rank, world, K, W, moments=args.moments)
+    copy_now = copy_bandwidth(dev) if world == 1 else None
     extras = []
     if args.config == 3 and precision == "f64" and world == 1 and not (args.no_extras or args.inplace or args.unfused or args.cpt or args.block or args.moments):
         # the fp32 instance of config 5 (BASELINE.json configs[4]) in the same run: device-resident throughput only
@@ -391,6 +412,9 @@ def run_acm(args, rank, local_rank, world):
     if rank == 0:
         p, N, esz, ms = r["p"], r["N"], r["esz"], r["ms"]
         roof, step_gbs, peak = roofline_of(args, args.config, precision, r, K)
+        if copy_now:
+            roof["copy_GBps_this_run"] = copy_now
+            roof["frac_of_copy_this_run"] = roof["achieved"] / copy_now
         out = {
             "metric": METRIC, "value": r["value"], "value_min": r["value_min"], "value_max": r["value_max"], "unit": UNIT, "n_gpus": world,
             "steps": K, "warmup": W, "repeats": REPEATS, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
