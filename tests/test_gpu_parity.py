@@ -359,7 +359,9 @@ def test_laplace_law_gpu():
 
 
 @pytest.mark.parametrize("mode", [dict(), dict(inplace=True), dict(unfused=True), dict(precision="f32"), dict(phase_srt=True),
-                                  dict(cpt=(2, 2)), dict(cpt=(2, 2), inplace=True), dict(cpt=(1, 1), precision="f32", inplace=True)])
+                                  dict(cpt=(2, 2)), dict(cpt=(2, 2), inplace=True), dict(cpt=(1, 1), precision="f32", inplace=True),
+                                  dict(moments=True, moment_kernels=(0, 0)), dict(moments=True, moment_kernels=(1, 0)),
+                                  dict(moments=True, moment_kernels=(1, 2))])
 @pytest.mark.parametrize("shape,Qh,Qg,walls", [((150, 7, 5), 15, 19, 0), ((33, 5, 4), 27, 27, inputs.WALL_X | inputs.WALL_Y | inputs.WALL_Z),
                                                ((260, 3, 2), 19, 27, inputs.WALL_Y), ((96, 50, 1), 9, 9, 0),
                                                ((36, 6, 11), 27, 27, inputs.WALL_X | inputs.WALL_Z)])
@@ -372,13 +374,17 @@ def test_no_write_outside_the_workspace(shape, Qh, Qg, walls, mode):
     u[2] = 0.0 if Qh == 9 else u[2]
     kw = dict(mode)
     cpt = kw.pop("cpt", None)      # force the pair / single-cell kernels where the grid allows (else the default stays)
+    mk = kw.pop("moment_kernels", None)      # moment representation: direct / tiled kernels, planes per block
     dt = np.float32 if kw.get("precision") == "f32" else np.float64
     a = ACM.from_params(p, guard_bytes=1 << 20, **kw)
     if cpt and (cpt == (1, 1) or p.nx % 2 == 0):
         a.set_cells_per_thread(*cpt)
     dev = lambda x: torch.from_numpy(np.ascontiguousarray(x, dtype=dt)).cuda()
+    if mk:
+        a.set_moment_kernels(*mk)
     a.init(dev(phi), dev(u))
-    a.set_pdfs(dev(h), dev(g))
+    if not mk:
+        a.set_pdfs(dev(h), dev(g))
     a.step(3)
     a.get_pdfs()
     a.fields()
