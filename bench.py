@@ -59,6 +59,10 @@ def workload(config, size=None):
     elif config == 7:
         p, phi, u = inputs.disc2d() if size is None else inputs.disc2d(n=size, count=4, r_min=size / 16, r_max=size / 8)
         name = f"2-D instance: {p.nx}^2 periodic, seeded discs + velocity noise, D2Q9+D2Q9 (P:360)"
+    elif config == 8:
+        # beyond what the population storage holds on one B200 (768^3 x 632 B = 286 GB): moment representation only (149 GB)
+        p, phi, u = inputs.config4(n=768, count=1728)
+        name = "768^3 periodic (453 M cells), 1728 seeded bubbles, D3Q15+D3Q19: the density of config 4 on the largest cube of 256-multiples that fits 180 GB in moment representation"
     elif config == 6:
         p, phi, u = inputs.paper_benchmark() if size is None else inputs.paper_benchmark(n=size)
         name = f"paper benchmark P:283: {p.nx}^3 periodic, one bubble R={p.nx // 4}, D3Q15 SRT + D3Q27 MRT"
@@ -387,7 +391,9 @@ def run_acm(args, rank, local_rank, world):
 
     K, W = args.steps, max(args.warmup, 20)      # never fewer than 20 warm-up steps
     precision = args.precision
-    r = measure(args, args.config, precision, dev, local_rank, world, K, W, moments=args.moments)
+    if args.config == 8 and not args.moments:
+        raise SystemExit("bench.py: --config 8 (768^3) needs --moments: the population storage would take 286 GB")
+    r = measure(args, args.config, precision, dev, local_rank, world, K, W, moments=args.moments, with_e2e=args.config != 8)
     copy_now = copy_bandwidth(dev) if world == 1 else None
     extras = []
     if args.config == 3 and precision == "f64" and world == 1 and not (args.no_extras or args.inplace or args.unfused or args.cpt or args.block or args.moments):
@@ -427,14 +433,14 @@ def run_acm(args, rank, local_rank, world):
                        "timing": f"median of {REPEATS} back-to-back intervals of {K} steps (CUDA events, no per-kernel instrumentation inside); "
                                  f"value_min / value_max = slowest / fastest interval; kernel split from a separate instrumented pass",
                        "interval_ms": r["intervals"],
-                       "l2": f"inputs larger than L2: {(2 * (p.stencil_phase + p.stencil_hydro) + 5) * N * esz / 1e9:.1f} GB "
+                       "l2": f"inputs larger than L2: {((2 * 14 + 8) if args.moments else (2 * (p.stencil_phase + p.stencil_hydro) + 5)) * N * esz / 1e9:.1f} GB "
                              "of state streamed every step vs 126 MB L2",
                        "bytes_per_cell": {"phase": r["b_phase"], "hydro": r["b_hydro"]},
                        "step_algorithmic_GBps": step_gbs, "step_frac_of_peak": step_gbs / peak, "step_frac_of_nominal": step_gbs / NOMINAL_HBM_GBS,
                        "phase_ms": r["phase_ms"], "hydro_ms": r["hydro_ms"], "cuda_graph_replays": r["graph_replays"],
-                       "sum_phi": r["mass"], "finite": r["finite"]},
+                       "sum_phi": r["mass"], "finite": r.get("finite")},
             "clocks": r["clocks"],
-            "e2e": {"value": r["e2e"], "unit": UNIT, "h2d_bytes_per_step": 4 * N * esz / K,
+            "e2e": {"value": r.get("e2e"), "unit": UNIT, "h2d_bytes_per_step": 4 * N * esz / K,
                     "d2h_bytes_per_step": 5 * N * esz / K, "steps": K,
                     "what": "acm_run_host: pinned host phi,u -> device, init, K steps, fields, phi,u,p -> host"},
             "gpu_launches": r["launches"],
